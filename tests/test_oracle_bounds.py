@@ -1,0 +1,130 @@
+"""Oracle pins II: brute-force hindsight optimum on tiny burst instances (config 1), the paper's
+bounds (Thm 3.2, Prop. 3.1, Lemma G.1, Lemma G.2, Thm 3.3) and the independent validator."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle import validator as V
+from paper_2606_22327_b200 import traces as T
+
+
+def _enumerate_opt(s, o, M):
+    """Plain enumeration of all start-time vectors (no search tricks) for n <= 4."""
+    n = len(s)
+    H = int(sum(o))                      # a left-shifted schedule never starts later than this
+    best = None
+    for ks in itertools.product(range(H + 1), repeat=n):
+        cost = sum(k + oi for k, oi in zip(ks, o))
+        if best is not None and cost >= best:
+            continue
+        ok = True
+        for t in range(1, H + max(o) + 1):
+            mem = sum(si + t - k for si, oi, k in zip(s, o, ks) if k < t <= k + oi)
+            if mem > M:
+                ok = False
+                break
+        if ok:
+            best = cost
+    return best
+
+
+def test_bruteforce_dfs_equals_plain_enumeration(oracle):
+    rng = np.random.default_rng(5)
+    for _ in range(25):
+        n = int(rng.integers(2, 5))
+        s = rng.integers(0, 5, size=n)
+        o = rng.integers(1, 4, size=n)
+        M = int(max(s + o) + rng.integers(0, 6))
+        opt, start, _ = oracle.bruteforce_opt(s, o, M)
+        assert opt == _enumerate_opt(list(map(int, s)), list(map(int, o)), M)
+        tr = T._one("x", np.zeros(n, np.int32), s, o, np.zeros(n, np.uint8), M, 1, 1)
+        info = V.validate(tr, 0, start, check_greedy=False)   # OPT need not be greedy
+        assert info["total_latency"] == opt
+
+
+N_SEEDS = 400
+
+
+def test_config1_policies_vs_optimum_and_paper_bounds(oracle):
+    """BASELINE.json configs[0]: n=8, burst, s,o ~ U{1..8}, M=32 (alpha <= 1/2)."""
+    worst = 0.0
+    n_opt_hit = 0
+    for inst in range(N_SEEDS):
+        tr = T.config1(inst)
+        s, o = tr.prompt.astype(np.int64), tr.output.astype(np.int64)
+        M = tr.M
+        opt, _, nodes = oracle.bruteforce_opt(s, o, M)
+        assert nodes < 5_000_000
+        vol = s * o + o * (o + 1) // 2
+        pmax = int((s + o).max())
+        # Lemma G.1 and Prop. 3.1 hold for OPT itself
+        assert opt >= int(o.sum())
+        assert M * opt >= int(np.cumsum(np.sort(vol)).sum())
+        tel = {}
+        for policy in range(4):
+            r = oracle.simulate(tr, policy)
+            assert r.status[0] == 0
+            tel[policy] = int(r.total_latency[0])
+            assert tel[policy] >= opt                                    # OPT is a lower bound
+            assert tel[policy] >= int(o.sum())                           # Lemma G.1
+            assert M * tel[policy] >= int(np.cumsum(np.sort(vol)).sum())  # Prop. 3.1
+            info = V.validate(tr, policy, r.start, finish=r.finish)
+            for f in ("total_latency", "peak_kv", "makespan", "p99_latency", "rounds", "decisions"):
+                assert info[f] == int(getattr(r, f)[0]), f
+        # Thm 3.2: TEL(SVF) <= (1 + 2/(1-alpha)) OPT, alpha = pmax/M, in integers
+        assert tel[0] * (M - pmax) <= opt * (3 * M - pmax)
+        # Thm 3.3: 1-bit SVF <= (9T+1) OPT with T = 16 >= max(s+o); loose
+        assert tel[1] <= (9 * 16 + 1) * opt
+        worst = max(worst, tel[0] / opt)
+        n_opt_hit += tel[0] == opt
+        # Lemma G.2, integer form: W_j == 0 or W_j (M - pmax) < 2 sum_{i in P_j} vol_i
+        r = oracle.simulate(tr, 0)
+        order = np.lexsort((np.arange(len(s)), vol))
+        pre = np.concatenate([[0], np.cumsum(vol[order])[:-1]])
+        W = r.start[order].astype(np.int64)
+        assert np.all((W == 0) | (W * (M - pmax) < 2 * pre))
+    assert worst <= 5.0 and n_opt_hit > N_SEEDS // 10
+
+
+@pytest.mark.parametrize("policy", [0, 1, 2, 3])
+@pytest.mark.parametrize("seed", range(6))
+def test_validator_accepts_oracle_on_random_online_instances(oracle, policy, seed):
+    tr = T.random_small(300 + seed, 60, 12, 10, M=50, a_hi=(0 if seed % 3 == 0 else 40))
+    r = oracle.simulate(tr, policy)
+    info = V.validate(tr, policy, r.start, finish=r.finish)
+    for f in ("total_latency", "peak_kv", "makespan", "p99_latency", "rounds", "decisions"):
+        assert info[f] == int(getattr(r, f)[0]), f
+    assert info["peak_kv"] <= tr.M
+
+
+def test_validator_rejects_wrong_schedules(oracle):
+    tr = T.random_small(42, 30, 10, 8, M=40)
+    r = oracle.simulate(tr, 0)
+    waited = np.nonzero(r.start > 0)[0]
+    assert len(waited) > 3
+    bad = r.start.copy()
+    bad[waited[-1]] = 0                     # start a blocked request early -> over capacity
+    with pytest.raises(AssertionError):
+        V.validate(tr, 0, bad)
+    late = r.start.copy()
+    late[np.argmin(r.start)] += 50          # delay the first request: bypass / idle head
+    with pytest.raises(AssertionError):
+        V.validate(tr, 0, late)
+    with pytest.raises(AssertionError):     # SVF schedule is not an FCFS-greedy schedule
+        V.validate(tr, 3, r.start)
+
+
+def test_config2_oracle_against_validator(oracle):
+    """BASELINE.json configs[1]: n=2000 online trace, M=300k; SVF vs SJF vs FCFS (+1-bit)."""
+    tr = T.config2()
+    tel = {}
+    for policy in range(4):
+        r = oracle.simulate(tr, policy)
+        assert r.status[0] == 0
+        info = V.validate(tr, policy, r.start, finish=r.finish, check_blocked=40)
+        for f in ("total_latency", "peak_kv", "makespan", "p99_latency", "rounds", "decisions"):
+            assert info[f] == int(getattr(r, f)[0]), f
+        tel[policy] = info["total_latency"]
+        assert info["blocked_checked"] > 0
+    assert tel[0] >= int(tr.output.astype(np.int64).sum())

@@ -1,0 +1,264 @@
+"""Pins for the CPU oracle (oracle/svf_ref.c): things the paper and the mathematics fix, none of
+them produced by the oracle itself or by the CUDA path.  CPU only (-m "not gpu")."""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from paper_2606_22327_b200 import traces as T
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+POL = {"svf": 0, "svf_1bit": 1, "sjf": 2, "fcfs": 3}
+
+
+# --------------------------------------------------------------------------------------------
+# P1: keys -- closed form Eq. 1 against the per-step memory of Eq. 3c
+# --------------------------------------------------------------------------------------------
+def test_volume_closed_form_equals_staircase_sum(oracle):
+    ss, oo = np.meshgrid(np.arange(0, 65), np.arange(1, 65), indexing="ij")
+    s, o = ss.ravel().astype(np.int32), oo.ravel().astype(np.int32)
+    rc, words = oracle.keys(oracle.SVF, s, o)
+    assert rc == 0
+    # the area a request occupies: s + j tokens at its j-th step, j = 1..o
+    expect = np.array([sum(int(si) + j for j in range(1, int(oi) + 1)) for si, oi in zip(s, o)],
+                      dtype=np.uint64)
+    assert np.array_equal(words >> np.uint64(32), expect)
+    assert np.array_equal(words & np.uint64(0xFFFFFFFF), np.arange(len(s), dtype=np.uint64))
+
+
+def test_proxy_volume_and_comparator_keys(oracle):
+    s = np.array([5, 0, 7, 7], dtype=np.int32)
+    o = np.array([3, 9, 1, 2], dtype=np.int32)
+    a = np.array([0, 2, 2, 11], dtype=np.int32)
+    bit = np.array([0, 1, 1, 0], dtype=np.uint8)
+    rc, w = oracle.keys(oracle.SVF_1BIT, s, o, a, bit, 2, 8)
+    # Eq. 2: s*O_m + (O_m^2+O_m)/2 with O_0=2 -> s*2+3, O_1=8 -> s*8+36
+    assert rc == 0 and list(w >> np.uint64(32)) == [5 * 2 + 3, 0 * 8 + 36, 7 * 8 + 36, 7 * 2 + 3]
+    rc, w = oracle.keys(oracle.SJF, s, o, a, bit, 2, 8)
+    assert list(w >> np.uint64(32)) == [3, 9, 1, 2]
+    rc, w = oracle.keys(oracle.FCFS, s, o, a, bit, 2, 8)
+    assert list(w >> np.uint64(32)) == [0, 2, 2, 11]
+    # key >= 2^32 is reported, not wrapped silently
+    rc, _ = oracle.keys(oracle.SVF, np.array([65536], np.int32), np.array([65536], np.int32))
+    assert rc == oracle.EOVERFLOW
+    # 1-bit needs the bit array and proxies >= 1
+    assert oracle.keys(oracle.SVF_1BIT, s, o, a, None, 2, 8)[0] == oracle.EINVAL
+    assert oracle.keys(oracle.SVF_1BIT, s, o, a, bit, 0, 8)[0] == oracle.EINVAL
+
+
+@pytest.mark.parametrize("T_, b", [(16, 2), (81, 3), (256, 4)])
+def test_eq35_sandwich_under_thm33_recipe(oracle, T_, b):
+    """Eq. 35: v_hat / b^2 <= vol <= b^2 v_hat with theta = sqrt(T), O_0 = T^(1/4),
+    O_1 = T^(3/4) (Thm 3.3), for every (s, o) with s + o <= T."""
+    theta, O0, O1 = b * b, b, b ** 3
+    so = [(s, o) for s in range(0, T_) for o in range(1, T_ + 1 - s)]
+    s = np.array([x[0] for x in so], np.int32)
+    o = np.array([x[1] for x in so], np.int32)
+    bit = (o > theta).astype(np.uint8)
+    vol = oracle.keys(oracle.SVF, s, o)[1] >> np.uint64(32)
+    vhat = oracle.keys(oracle.SVF_1BIT, s, o, None, bit, O0, O1)[1] >> np.uint64(32)
+    b2 = np.uint64(b * b)
+    assert np.all(vhat <= b2 * vol) and np.all(vol <= b2 * vhat)
+
+
+def test_table1_constants():
+    """Table 1: 1 + 2/(1-alpha) = 5.00, 3.67, 3.22, 3.11, 3.02."""
+    golden = {}
+    for line in open(os.path.join(GOLDEN, "table1.txt")):
+        if line.strip() and not line.startswith("#"):
+            den, val = line.split()
+            golden[int(den)] = float(val)
+    assert set(golden) == {2, 4, 10, 20, 100}
+    for den, val in golden.items():
+        assert round(1 + 2 / (1 - 1 / den), 2) == val
+
+
+# --------------------------------------------------------------------------------------------
+# P2: literal FEASIBLE (Eq. 3c at every future step) == completion-time form
+# --------------------------------------------------------------------------------------------
+def test_feasible_literal_equals_completion_form(oracle):
+    rng = np.random.default_rng(12345)
+    n_true = 0
+    for _ in range(20000):
+        m = int(rng.integers(0, 9))
+        kv = rng.integers(0, 12, size=m)
+        rem = rng.integers(1, 10, size=m)
+        # M near the peak so that both outcomes occur
+        peak_guess = int((kv + rem).sum()) if m else 0
+        M = int(rng.integers(max(0, peak_guess // 2), peak_guess + 2))
+        lit = oracle.feasible(kv, rem, M, oracle.FEAS_LITERAL)
+        com = oracle.feasible(kv, rem, M, oracle.FEAS_COMPLETION)
+        assert lit == com
+        # and against a third, direct statement in Python
+        direct = all(sum(int(kv[i]) + d for i in range(m) if rem[i] >= d) <= M
+                     for d in range(1, (int(rem.max()) if m else 0) + 1))
+        assert lit == direct
+        n_true += lit
+    assert 2000 < n_true < 18000   # both outcomes exercised
+
+
+def test_feasible_boundary_is_inclusive(oracle):
+    # one request (kv=3, rem=4) peaks at 3+4=7 at its last step: feasible iff M >= 7 ("<=", Eq. 3c)
+    assert oracle.feasible([3], [4], 7) and not oracle.feasible([3], [4], 6)
+    assert oracle.feasible([3], [4], 7, oracle.FEAS_LITERAL)
+    assert not oracle.feasible([3], [4], 6, oracle.FEAS_LITERAL)
+    assert oracle.feasible([], [], 0)
+
+
+# --------------------------------------------------------------------------------------------
+# P4: hand-derived micro-examples (tests/golden/hand_examples.txt)
+# --------------------------------------------------------------------------------------------
+def _load_examples():
+    ex, cur = [], None
+    for line in open(os.path.join(GOLDEN, "hand_examples.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        tok = line.split()
+        if tok[0] == "example":
+            cur = {"name": tok[1], "M": int(tok[2].split("=")[1]),
+                   "policy": POL[tok[3].split("=")[1]], "req": []}
+            ex.append(cur)
+        elif tok[0] == "req":
+            cur["req"].append(tuple(int(x) for x in tok[1:4]))
+        elif tok[0] == "start":
+            cur["start"] = [int(x) for x in tok[1:]]
+        elif tok[0] == "tel":
+            cur["tel"] = int(tok[1])
+    return ex
+
+
+@pytest.mark.parametrize("ex", _load_examples(), ids=lambda e: e["name"])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_hand_examples(oracle, ex, mode):
+    a, s, o = (np.array(x, np.int32) for x in zip(*ex["req"]))
+    tr = T._one(ex["name"], a, s, o, np.zeros(len(a), np.uint8), ex["M"], 1, 1)
+    r = oracle.simulate(tr, ex["policy"], mode=mode)
+    assert r.status[0] == 0
+    assert list(r.start) == ex["start"]
+    assert list(r.finish) == [k + int(oi) for k, oi in zip(ex["start"], o)]
+    assert int(r.total_latency[0]) == ex["tel"]
+
+
+# --------------------------------------------------------------------------------------------
+# P5: degenerate reductions
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("policy", [0, 1, 2, 3])
+def test_unbounded_memory_starts_everything_on_arrival(oracle, policy):
+    tr = T.random_small(7, 60, 20, 15, M=10 ** 6, a_hi=25)
+    r = oracle.simulate(tr, policy)
+    assert np.array_equal(r.start, tr.arrival)
+    assert int(r.total_latency[0]) == int(tr.output.sum())          # Lemma G.1 tight
+    assert int(r.rounds[0]) == len(np.unique(tr.arrival))
+    assert int(r.decisions[0]) == tr.n_requests
+
+
+@pytest.mark.parametrize("s,o,m,r_", [(3, 4, 2, 0), (3, 4, 2, 3), (0, 5, 3, 0), (5, 1, 4, 2)])
+def test_identical_requests_run_in_pure_batches(oracle, s, o, m, r_):
+    """n identical (s, o), burst, M = m(s+o) + r, 0 <= r <= s: exactly m fit (each peaks at s+o
+    in lockstep), so batch b (0-based) has latency (b+1) o."""
+    n = 3 * m + 1
+    M = m * (s + o) + r_
+    tr = T._one("ident", np.zeros(n, np.int32), np.full(n, s, np.int32), np.full(n, o, np.int32),
+                np.zeros(n, np.uint8), M, 1, 1)
+    for policy in range(4):
+        r = oracle.simulate(tr, policy)
+        assert list(r.start) == [(i // m) * o for i in range(n)]
+        assert int(r.total_latency[0]) == sum(((i // m) + 1) * o for i in range(n))
+        assert int(r.peak_kv[0]) == m * (s + o)
+
+
+def test_unit_outputs_reduce_to_prefix_packing(oracle):
+    """all o_i = 1: each step admits the longest sorted prefix with sum (s_i + 1) <= M."""
+    tr = T.random_small(11, 40, 9, 1, M=23)
+    r = oracle.simulate(tr, oracle.SVF)
+    order = np.lexsort((np.arange(40), tr.prompt.astype(np.int64) + 1))   # vol = s + 1
+    t, i, expect = 0, 0, np.zeros(40, np.int64)
+    while i < 40:
+        load = 0
+        while i < 40 and load + tr.prompt[order[i]] + 1 <= 23:
+            load += tr.prompt[order[i]] + 1
+            expect[order[i]] = t
+            i += 1
+        t += 1
+    assert np.array_equal(r.start, expect)
+
+
+def test_policy_coincidences(oracle):
+    # equal prompts: volume is increasing in o, so SVF == SJF
+    tr = T.random_small(3, 50, 0, 12, M=40)
+    tr.prompt[:] = 6
+    assert np.array_equal(oracle.simulate(tr, oracle.SVF).start, oracle.simulate(tr, oracle.SJF).start)
+    # all keys equal: every policy is FCFS (ties broken by arrival then id)
+    tr = T.random_small(4, 50, 0, 1, M=30, a_hi=10)
+    tr.prompt[:] = 4
+    tr.output[:] = 5
+    tr.bit[:] = 1
+    ref = oracle.simulate(tr, oracle.FCFS).start
+    for p in (oracle.SVF, oracle.SVF_1BIT, oracle.SJF):
+        assert np.array_equal(oracle.simulate(tr, p).start, ref)
+    # all bits equal: 1-bit SVF orders by prompt size
+    tr = T.random_small(5, 30, 10, 6, M=40)
+    tr.bit[:] = 0
+    r = oracle.simulate(tr, oracle.SVF_1BIT)
+    order = np.lexsort((np.arange(30), tr.prompt))
+    assert np.all(np.diff(r.start[order]) >= 0)
+
+
+# --------------------------------------------------------------------------------------------
+# literal and completion-time simulators agree; invalid inputs are rejected
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(12))
+def test_simulator_literal_equals_completion(oracle, seed):
+    tr = T.random_small(100 + seed, 40, 10, 9, M=45, a_hi=(0 if seed % 2 else 30))
+    for policy in range(4):
+        r0 = oracle.simulate(tr, policy, mode=0)
+        r1 = oracle.simulate(tr, policy, mode=1)
+        for f in ("start", "finish", "total_latency", "p99_latency", "makespan", "peak_kv",
+                  "rounds", "decisions", "status"):
+            assert np.array_equal(getattr(r0, f), getattr(r1, f)), f
+
+
+def test_invalid_instances_get_status_codes(oracle):
+    def run(a, s, o, M=100, policy=0):
+        tr = T._one("bad", np.array(a, np.int32), np.array(s, np.int32), np.array(o, np.int32),
+                    np.zeros(len(a), np.uint8), M, 1, 1)
+        return int(oracle.simulate(tr, policy).status[0])
+    assert run([0, 1], [1, 1], [1, 1]) == oracle.OK
+    assert run([0, 1], [1, 1], [0, 1]) == oracle.ERANGE
+    assert run([0, 1], [-1, 1], [1, 1]) == oracle.ERANGE
+    assert run([2, 1], [1, 1], [1, 1]) == oracle.EUNSORTED
+    assert run([0, 1], [60, 1], [41, 1]) == oracle.EINFEASIBLE
+    assert run([0, 2 ** 31 - 5], [1, 1], [3, 3], M=10) == oracle.EOVERFLOW
+    assert run([0], [70000], [70000], M=10 ** 9) == oracle.EOVERFLOW
+    # lowest-numbered failing check wins
+    assert run([2, 1], [1, 1], [0, 1]) == oracle.ERANGE
+    # a failing instance does not disturb its neighbours
+    good = T.random_small(1, 10, 5, 5, M=30)
+    bad = T._one("bad", np.array([3, 1], np.int32), np.array([1, 1], np.int32),
+                 np.array([1, 1], np.int32), np.zeros(2, np.uint8), 30, 1, 1)
+    both = T.concat([good, bad, good], "mix", 30, 2, 8)
+    r = oracle.simulate(both, 0)
+    assert list(r.status) == [0, oracle.EUNSORTED, 0]
+    assert np.array_equal(r.start[:10], r.start[12:]) and np.all(r.start[10:12] == -1)
+    assert r.total_latency[0] == r.total_latency[2] > 0 and r.total_latency[1] == 0
+
+
+# --------------------------------------------------------------------------------------------
+# stateless admit == what the simulator does at a step
+# --------------------------------------------------------------------------------------------
+def test_admit_matches_simulator_first_step(oracle):
+    for seed in range(20):
+        tr = T.random_small(200 + seed, 30, 10, 9, M=60)
+        for policy in range(4):
+            sim = oracle.simulate(tr, policy)
+            rc, idx, words = oracle.admit(policy, tr.M, 0, tr.prompt, tr.output, tr.arrival,
+                                          tr.bit, tr.O0, tr.O1, [], [])
+            assert rc == 0
+            assert sorted(idx.tolist()) == np.nonzero(sim.start == 0)[0].tolist()
+            assert np.all(np.diff(words.astype(object)) > 0)
+            assert np.array_equal(words[: len(idx)] & np.uint64(0xFFFFFFFF), idx.astype(np.uint64))
+            rc2, idx2, _ = oracle.admit(policy, tr.M, 0, tr.prompt, tr.output, tr.arrival,
+                                        tr.bit, tr.O0, tr.O1, [], [], mode=0)
+            assert np.array_equal(idx, idx2)
