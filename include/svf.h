@@ -1,0 +1,147 @@
+/*
+ * include/svf.h -- C ABI of libsvf_b200: the data-parallel hot path of "Geometry-Aware Online
+ * Scheduling for LLM Serving" (arxiv/paper_2606_22327), hand-written CUDA for sm_100a.
+ *
+ * Citations: "P:L<n>" = line n of the paper text; "R<k>" = reading k of DESIGN.md 3.
+ *
+ * The model (Eq. 3a-3d): discrete time, KV budget M, request i = (a_i, s_i, o_i) =
+ * (arrival step, prompt tokens, output tokens).  Started at k_i >= a_i it holds s_i + (t - k_i)
+ * tokens at every t in {k_i+1 .. k_i+o_i} (Eq. 3c), finishes at f_i = k_i + o_i with latency
+ * f_i - a_i, is never preempted; sum of held tokens <= M at every t.
+ * The policy: order the waiting queue by ascending key --
+ * volume v_i = s_i o_i + (o_i^2 + o_i)/2 (Eq. 1), proxy volume s_i O_m + (O_m^2 + O_m)/2 with
+ * m = bit_i (Eq. 2), o_i (SJF) or a_i (FCFS) -- ties broken by (arrival, id);
+ * admit the head while the forward-looking check passes (no future time exceeds M with it
+ * added); a blocked head is never bypassed.
+ *
+ * Conventions for every entry point
+ *  - DEVICE pointers are marked [dev]; HOST pointers [host].  The caller owns every buffer; the
+ *    library allocates nothing and keeps no global state.  Scratch comes from the caller (`ws`,
+ *    [dev], 256-byte aligned, size from the matching *_workspace_bytes call).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls only
+ *    enqueue work; outputs are valid once the stream has been synchronised.
+ *  - Return value: svf_status_t for errors the HOST can see (arguments, sizes, CUDA launch
+ *    errors).  Errors that depend on the DATA are found on the device and written to a status
+ *    word ([dev], per instance for svf_simulate); they are never undefined behaviour and one
+ *    instance's error does not disturb the others.
+ *  - All arithmetic is integer and exact; there is no CPU fallback: without a CUDA device every
+ *    compute call returns SVF_ECUDA.
+ */
+#ifndef SVF_H_
+#define SVF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Priority rule. */
+typedef enum { SVF_SVF = 0, SVF_SVF_1BIT = 1, SVF_SJF = 2, SVF_FCFS = 3 } svf_policy_t;
+
+typedef enum {
+    SVF_OK = 0,
+    SVF_EINVAL = 1,       /* host: null pointer, negative size, unknown policy, O0/O1 < 1, missing bit */
+    SVF_EWORKSPACE = 2,   /* host: ws is NULL or ws_bytes too small                                   */
+    SVF_ECUDA = 3,        /* host: no device / launch failed (cudaGetLastError != success)           */
+    SVF_ERANGE = 16,      /* data: o_i < 1, s_i < 0 or a_i < 0 (running set: rem < 1 or kv < 0)        */
+    SVF_EUNSORTED = 17,   /* data: arrivals decrease inside an instance                              */
+    SVF_EINFEASIBLE = 18, /* data: s_i + o_i > M, could never be admitted (paper assumes <= aM) */
+    SVF_EOVERFLOW = 19    /* data: key >= 2^32, or max a + sum o >= 2^31 (horizon bound)       */
+} svf_status_t;
+/* When several data checks fail in one instance the lowest-numbered code is reported. */
+
+/* A batch of independent instances ("n requests ... global capacity M"), SoA, instances
+ * concatenated.  Instance j is the index range [offsets[j], offsets[j+1]); inside it requests
+ * are in (arrival, id) order, i.e. arrivals are non-decreasing and the local index is the id. */
+typedef struct {
+    int64_t        n_instances;   /* [host] I >= 0                                                  */
+    int64_t        n_requests;    /* [host] N = offsets[I], 0 <= N < 2^30                           */
+    int64_t        max_instance;  /* [host] max_j (offsets[j+1]-offsets[j]); sizes the on-chip state */
+    const int64_t* offsets;       /* [dev] [I+1], offsets[0] = 0, non-decreasing                    */
+    const int32_t* arrival;       /* [dev] [N] a_i >= 0                                             */
+    const int32_t* prompt;        /* [dev] [N] s_i >= 0                                             */
+    const int32_t* output;        /* [dev] [N] o_i >= 1 (true length: drives dynamics AND the check, R7) */
+    const uint8_t* bit;           /* [dev] [N] 0 = short, 1 = long; may be NULL unless SVF_SVF_1BIT */
+    int32_t        O0, O1;        /* [host] integer proxy lengths of Eq. 2 (>= 1 for SVF_SVF_1BIT)   */
+} svf_trace_t;
+
+/* Caller-allocated DEVICE outputs of svf_simulate.  Any pointer may be NULL (not wanted). */
+typedef struct {
+    int32_t* start;          /* [dev] [N] k_i  (-1 for requests of a rejected instance)            */
+    int32_t* finish;         /* [dev] [N] f_i = k_i + o_i (-1 likewise)                             */
+    int64_t* total_latency;  /* [dev] [I] sum_i (f_i - a_i)            (Eq. 3a)              */
+    int64_t* p99_latency;    /* [dev] [I] nearest-rank: ceil(0.99 n)-th smallest latency (R13)      */
+    int32_t* makespan;       /* [dev] [I] max_i f_i                                                 */
+    int64_t* peak_kv;        /* [dev] [I] max_t mem(t) by Eq. 3c (always <= M)                      */
+    int64_t* rounds;         /* [dev] [I] steps whose queue is non-empty after arrivals (R16)       */
+    int64_t* decisions;      /* [dev] [I] admissions + one blocked-head evaluation per round that
+                                          ends with a non-empty queue (R16)                         */
+    int32_t* status;         /* [dev] [I] SVF_OK or a data error; a rejected instance reports zeros */
+} svf_result_t;
+
+/* a1 + a2 (Eq. 1 / Eq. 2 / SJF / FCFS): words_out[i] = (key_i << 32) + i,
+ * i = index in the (arrival, id)-ordered input, so ascending word order IS the priority order
+ * (key, arrival, id).  s, o: [dev][n]; a: [dev][n], needed for SVF_FCFS only (else may be NULL);
+ * bit: [dev][n], needed for SVF_SVF_1BIT only.  status_out: [dev] one int32, set to SVF_OK or
+ * SVF_EOVERFLOW (some key >= 2^32; that word holds the key modulo 2^32); may be NULL.
+ * 0 <= n <= 2^32.  One streaming pass: 8-13 B read + 8 B written per request. */
+int svf_keys(int policy, int64_t n, const int32_t* s, const int32_t* o, const int32_t* a,
+             const uint8_t* bit, int32_t O0, int32_t O1, uint64_t* words_out,
+             int32_t* status_out, void* stream);
+
+/* a1-a5: one stateless admission decision.
+ * Waiting requests [dev][n_wait] (w_s, w_o, w_a, w_bit) in (arrival, id) order; running
+ * requests [dev][n_run] as r_kv (tokens held now) and r_rem (steps left, >= 1): r holds
+ * r_kv + d tokens d steps from now, d = 1..r_rem.  The call computes the keys, radix-sorts the
+ * packed words, and admits the longest prefix of the priority order whose members are jointly
+ * feasible with the running set (a request admitted now holds w_s + d tokens for d = 1..w_o),
+ * stopping at the first blocked head.  Outputs, all [dev]:
+ *   n_admitted_out    one int64: k
+ *   admitted_idx_out  [n_wait] int32: the first k entries are the admitted input indices in
+ *                     priority order (the rest is unspecified); may be NULL
+ *   sorted_words_out  [n_wait] uint64: the whole queue in priority order as (key << 32) + index;
+ *                     may be NULL
+ *   status_out        one int32: SVF_OK / SVF_ERANGE / SVF_EUNSORTED / SVF_EOVERFLOW; on error
+ *                     k = 0
+ * `t` only dates the decision (the check is relative to now).  0 <= n_wait, n_run < 2^30. */
+size_t svf_admit_workspace_bytes(int64_t n_wait, int64_t n_run);
+int svf_admit(int policy, int64_t M, int32_t t,
+              int64_t n_wait, const int32_t* w_s, const int32_t* w_o, const int32_t* w_a,
+              const uint8_t* w_bit, int32_t O0, int32_t O1,
+              int64_t n_run, const int32_t* r_kv, const int32_t* r_rem,
+              int64_t* n_admitted_out, int32_t* admitted_idx_out, uint64_t* sorted_words_out,
+              int32_t* status_out, void* ws, size_t ws_bytes, void* stream);
+
+/* a1-a7: the batched discrete-time simulator (P:L87-104 model; Alg. 1 Process 2).
+ * Per instance, from t = a_0:  COMPLETE (k_i + o_i == t) -> ARRIVE (a_i <= t) -> ADMIT (pop
+ * the head of the (key, arrival, id) order while the forward-looking check passes; stop at the
+ * first blocked head) -> t+1  (event order: R1), until every request has finished.
+ * Device-wide phase: validate + keys + one segmented onesweep radix sort giving every
+ * instance its priority order; then one persistent kernel, one thread group per instance.
+ * `trace` and `out` are HOST structs holding DEVICE pointers (see above). */
+size_t svf_simulate_workspace_bytes(const svf_trace_t* trace);
+int svf_simulate(const svf_trace_t* trace, int policy, int64_t M, const svf_result_t* out,
+                 void* ws, size_t ws_bytes, void* stream);
+
+/* The sort subsystem on its own (a3), for tests and measurement: ascending, stable LSD
+ * onesweep radix sort of n 64-bit words on the bit range [bit_lo, bit_hi) (0 <= bit_lo <
+ * bit_hi <= 64; words that agree on that range keep their input order).  words_in: [dev][n]
+ * (not modified); words_out: [dev][n].  0 <= n < 2^30. */
+size_t svf_sort_workspace_bytes(int64_t n, int bit_lo, int bit_hi);
+int svf_sort_words(int64_t n, const uint64_t* words_in, uint64_t* words_out, int bit_lo,
+                   int bit_hi, void* ws, size_t ws_bytes, void* stream);
+
+/* Number of kernels the last call of each kind enqueued on this host thread (for the
+ * "gpu_launches" count of bench.py); which: 0 = svf_keys, 1 = svf_admit, 2 = svf_simulate,
+ * 3 = svf_sort_words. */
+int64_t svf_last_launch_count(int which);
+
+const char* svf_status_string(int status);
+const char* svf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SVF_H_ */

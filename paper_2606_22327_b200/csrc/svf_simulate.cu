@@ -1,0 +1,482 @@
+// a1-a7: the batched discrete-time simulator of the paper's KV-cache model under the
+// SVF / 1-bit SVF / SJF / FCFS admission rule (Alg. 1 Process 2).
+//
+// Phase A (device-wide, HBM-bound):  k_sim_pack  keys (Eq. 1 / Eq. 2) packed as
+//     [ instance | key (32) | local id (sb) ]  ->  onesweep radix sort on [sb, sb+32+ib)
+//     (stable, input is in (instance, arrival, id) order, so the result is the
+//     (instance, key, arrival, id) order)  ->  k_sim_rank  order[] / rank[] per instance.
+// Phase B (persistent, on-chip):  k_sim  one thread group (warp or CTA) per instance, work
+//     handed out by an atomic counter; running set and waiting bitmap in shared memory (in an
+//     L2-resident workspace slot when an instance is too large), see svf_state.cuh.
+// Phase C:  p99 by one more onesweep sort of (instance, latency) words + k_sim_p99.
+//
+// Time advance is event driven but exact (R1, R16): steps on which nothing can happen are
+// jumped over -- an empty queue jumps to the next arrival/completion; a blocked head jumps to
+// the next arrival/completion or to the first step at which condition (2) of the check can
+// hold (it relaxes by exactly one token per step while the running set is unchanged) -- and
+// the skipped steps are still counted into rounds/decisions exactly as the step-by-step
+// definition counts them.
+#include <limits.h>
+
+#include "svf_internal.cuh"
+#include "svf_state.cuh"
+
+namespace svf {
+
+namespace {
+
+struct SimArgs {
+    int64_t I, N, M, max_instance;
+    int policy; int32_t O0, O1;
+    int sb;                          // bits of the local-id field
+    const int64_t* off;
+    const int32_t *a, *s, *o;
+    const uint8_t* bit;
+    const uint32_t* order;           // [N] local id at (instance offset + rank)
+    const uint32_t* rank;            // [N] rank of (instance offset + local id)
+    int32_t *start, *finish;
+    int64_t *tel, *peak, *rounds, *decisions;
+    int32_t *makespan, *status;
+    uint64_t* latw;                  // [N] (instance << 32) + latency, or NULL
+    unsigned long long* work_ctr;
+    char* gstate;                    // per-CTA state slots when the state is not in shared memory
+    size_t slot_bytes;
+    int cap;                         // entries per state slot
+};
+
+__host__ __device__ inline size_t state_bytes(int cap)
+{
+    int nL0 = (cap + 31) / 32, nL1 = (nL0 + 31) / 32;
+    return align_up((size_t)cap * 8, 16) + align_up((size_t)cap * 4, 16) + align_up((size_t)nL0 * 4, 16) +
+           align_up((size_t)nL1 * 4, 16);
+}
+
+// ---- Phase A ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_sim_pack(SimArgs g, uint64_t* __restrict__ words)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const uint64_t seq_mask = g.sb >= 64 ? ~0ull : ((1ull << g.sb) - 1ull);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < g.N; i += stride) {
+        // instance of request i: last j with off[j] <= i
+        int64_t lo = 0, hi = g.I - 1;
+        while (lo < hi) {
+            int64_t mid = (lo + hi + 1) >> 1;
+            if (__ldg(g.off + mid) <= i) lo = mid; else hi = mid - 1;
+        }
+        const int64_t seq = i - __ldg(g.off + lo);
+        const uint32_t b = g.policy == SVF_SVF_1BIT ? (uint32_t)__ldg(g.bit + i) : 0u;
+        const uint64_t key = priority_key(g.policy, __ldg(g.s + i), __ldg(g.o + i), __ldg(g.a + i), b, g.O0, g.O1);
+        words[i] = ((uint64_t)lo << (32 + g.sb)) | ((key & 0xffffffffull) << g.sb) | ((uint64_t)seq & seq_mask);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_sim_rank(SimArgs g, const SortPlan* __restrict__ plan,
+                                                  uint32_t* __restrict__ order, uint32_t* __restrict__ rank)
+{
+    const uint64_t* __restrict__ sorted = plan->result;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const uint64_t seq_mask = g.sb >= 64 ? ~0ull : ((1ull << g.sb) - 1ull);
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < g.N; p += stride) {
+        const uint64_t w = sorted[p];
+        const int64_t j = (int64_t)(w >> (32 + g.sb));
+        const int64_t seq = (int64_t)(w & seq_mask);
+        if (j >= g.I) continue;                       // only reachable with a corrupt layout
+        const int64_t base = __ldg(g.off + j);
+        const int64_t r = p - base;
+        order[p] = (uint32_t)seq;
+        if (r >= 0 && base + seq < g.N) rank[base + seq] = (uint32_t)r;
+    }
+}
+
+// ---- Phase B ---------------------------------------------------------------------------------
+template <int THREADS, bool SMEM>
+__global__ void __launch_bounds__(THREADS) k_sim(SimArgs g)
+{
+    using G = Group<THREADS>;
+    extern __shared__ __align__(16) char dyn_smem[];
+    __shared__ int scratch[2][64];
+    __shared__ long long inst_s;
+    int parity = 0;
+    const int tid = threadIdx.x, lane = tid & 31;
+
+    char* sbase = SMEM ? dyn_smem : g.gstate + (size_t)blockIdx.x * g.slot_bytes;
+    const int cap = g.cap;
+    const int capL0 = (cap + 31) / 32, capL1 = (capL0 + 31) / 32;
+    int64_t* A = reinterpret_cast<int64_t*>(sbase);
+    int32_t* f = reinterpret_cast<int32_t*>(sbase + align_up((size_t)cap * 8, 16));
+    uint32_t* L0 = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(f) + align_up((size_t)cap * 4, 16));
+    uint32_t* L1 = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(L0) + align_up((size_t)capL0 * 4, 16));
+
+    while (true) {
+        if (tid == 0) inst_s = (long long)atomicAdd(g.work_ctr, 1ull);
+        __syncthreads();
+        const int64_t j = inst_s;
+        __syncthreads();
+        if (j >= g.I) break;
+
+        const int64_t base = g.off[j];
+        const int64_t n64 = g.off[j + 1] - base;
+        uint32_t flags = 0;
+        if (n64 < 0 || n64 > g.max_instance || base < 0 || base + (n64 > 0 ? n64 : 0) > g.N ||
+            g.off[0] != 0 || g.off[g.I] != g.N)
+            flags |= F_LAYOUT;
+        const int n = (flags & F_LAYOUT) ? 0 : (int)n64;
+        const int32_t* __restrict__ a = g.a + base;
+        const int32_t* __restrict__ s = g.s + base;
+        const int32_t* __restrict__ o = g.o + base;
+
+        // ---- validation (data errors -> status[j], never UB) --------------------------------
+        int64_t sum_o = 0;
+        int max_a = 0;
+        for (int i = tid; i < n; i += THREADS) {
+            const int32_t ai = a[i], si = s[i], oi = o[i];
+            if (oi < 1 || si < 0 || ai < 0) flags |= F_RANGE;
+            if (i > 0 && ai < a[i - 1]) flags |= F_UNSORTED;
+            if ((int64_t)si + oi > g.M) flags |= F_INFEASIBLE;
+            const uint32_t b = g.policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
+            if (oi >= 1 && si >= 0 && ai >= 0 && (priority_key(g.policy, si, oi, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
+            sum_o += oi > 0 ? oi : 0;
+            max_a = ai > max_a ? ai : max_a;
+        }
+        flags = G::or_u32(flags, scratch, parity);
+        sum_o = G::sum_i64(sum_o, scratch, parity);
+        { int z = 0; G::sum_max(z, max_a, scratch, parity); }
+        if ((int64_t)max_a + sum_o >= ((int64_t)1 << 31)) flags |= F_OVERFLOW;   // horizon
+        const int32_t status = status_from_flags(flags);
+
+        int64_t tel = 0, peak = 0, rounds = 0, decisions = 0;
+        int32_t mk = 0;
+
+        if (status != SVF_OK || n == 0) {
+            const int nn = (flags & F_LAYOUT) ? 0 : (int)n64;
+            for (int i = tid; i < nn; i += THREADS) {
+                if (g.start) g.start[base + i] = -1;
+                if (g.finish) g.finish[base + i] = -1;
+                if (g.latw) g.latw[base + i] = (uint64_t)j << 32;
+            }
+        } else {
+            const uint32_t* __restrict__ order = g.order + base;
+            const uint32_t* __restrict__ rnk = g.rank + base;
+            const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
+            for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
+            for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
+            G::sync();
+
+            int R = 0, next = 0, started = 0;
+            int32_t t = a[0];
+            int hr = INT_MAX;                        // rank of the head of the queue
+            int32_t hid = 0, sh = 0, oh = 0;         // its id, s, o
+            bool head_loaded = false;
+
+            while (started < n) {
+                // 1. COMPLETE: entries with f == t are the tail of the array
+                while (R > 0) {
+                    const int jx = R - 1 - lane;
+                    const int32_t fj = jx >= 0 ? f[jx] : -1;
+                    const uint32_t m = __ballot_sync(FULL, fj == t);
+                    const int c = (m == FULL) ? 32 : (__ffs(~m) - 1);
+                    if (c > 0) { const int64_t Al = A[R - 1]; peak = Al > peak ? Al : peak; }
+                    R -= c;
+                    if (c < 32) break;
+                }
+                // 2. ARRIVE: a_i <= t join the queue (every warp tracks the count, warp 0 writes)
+                bool any_arrival = false;
+                while (next < n) {
+                    const int idx = next + lane;
+                    const bool v = idx < n && a[idx] <= t;
+                    const uint32_t m = __ballot_sync(FULL, v);
+                    const int c = __popc(m);
+                    int r = INT_MAX;
+                    if (v) { r = (int)rnk[idx]; if (tid < 32) queue_set(L0, L1, r); }
+                    r = __reduce_min_sync(FULL, r);
+                    if (r < hr) { hr = r; head_loaded = false; }
+                    next += c;
+                    any_arrival |= c > 0;
+                    if (c < 32) break;
+                }
+                if (any_arrival) G::sync();
+                // 3. ADMIT
+                int64_t wait = 1;
+                if (next > started) {
+                    rounds += 1;
+                    while (next > started) {
+                        if (!head_loaded) {
+                            hid = (int32_t)order[hr]; sh = s[hid]; oh = o[hid];
+                            head_loaded = true;
+                        }
+                        const Verdict v = evaluate_head<THREADS>(f, A, R, t, sh, oh, g.M, scratch, parity);
+                        if (!v.ok) { wait = v.wait; break; }
+                        insert_head<THREADS>(f, A, R, v.pos, t, sh, oh, v.Ah);
+                        ++R;
+                        const int32_t fh = t + oh;
+                        if (tid == 0) {
+                            queue_clear(L0, L1, hr);
+                            if (g.start) g.start[base + hid] = t;
+                            if (g.finish) g.finish[base + hid] = fh;
+                            if (g.latw) g.latw[base + hid] = ((uint64_t)j << 32) | (uint32_t)(fh - a[hid]);
+                        }
+                        tel += fh - a[hid];
+                        mk = fh > mk ? fh : mk;
+                        ++started; ++decisions;
+                        G::sync();
+                        head_loaded = false;
+                        hr = (next > started) ? queue_min(L0, L1, nL1, hr >> 10) : INT_MAX;
+                    }
+                    if (next > started) ++decisions;          // one blocked-head evaluation
+                }
+                if (started == n) break;
+                // 4. ADVANCE to the next step at which anything can change
+                const int64_t t_arr = next < n ? (int64_t)a[next] : (int64_t)INT_MAX;
+                const int64_t t_cmp = R > 0 ? (int64_t)f[R - 1] : (int64_t)INT_MAX;
+                int64_t tn = t_arr < t_cmp ? t_arr : t_cmp;
+                if (next > started) {                         // blocked head waits
+                    const int64_t t_lb = (int64_t)t + wait;
+                    tn = t_lb < tn ? t_lb : tn;
+                    rounds += tn - t - 1;
+                    decisions += tn - t - 1;
+                }
+                t = (int32_t)tn;
+            }
+            // drain: the remaining completions only matter for the peak
+            int64_t pk = 0;
+            for (int jx = tid; jx < R; jx += THREADS) { const int64_t Al = A[jx]; pk = Al > pk ? Al : pk; }
+            pk = G::max_i64_nonneg(pk, scratch, parity);
+            peak = pk > peak ? pk : peak;
+        }
+        if (tid == 0) {
+            if (g.tel) g.tel[j] = tel;
+            if (g.peak) g.peak[j] = peak;
+            if (g.rounds) g.rounds[j] = rounds;
+            if (g.decisions) g.decisions[j] = decisions;
+            if (g.makespan) g.makespan[j] = mk;
+            if (g.status) g.status[j] = status;
+        }
+        G::sync();
+    }
+}
+
+// ---- Phase C ---------------------------------------------------------------------------------
+__global__ void k_sim_p99(int64_t I, const int64_t* __restrict__ off, const SortPlan* __restrict__ plan,
+                          const int32_t* __restrict__ status, int64_t* __restrict__ p99)
+{
+    const uint64_t* __restrict__ sorted = plan->result;
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= I) return;
+    const int64_t base = off[j], n = off[j + 1] - base;
+    int64_t v = 0;
+    if (n > 0 && status[j] == SVF_OK) {
+        const int64_t rank = (99 * n + 99) / 100;       // nearest rank ceil(0.99 n), 1-based (R13)
+        v = (int64_t)(uint32_t)sorted[base + rank - 1];
+    }
+    p99[j] = v;
+}
+
+struct SimWs {
+    SortWs sort;            // sized for the larger of the two sorts
+    uint64_t* words0;       // [N]
+    uint64_t* words1;       // [N]
+    uint32_t* order;        // [N]
+    uint32_t* rank;         // [N]
+    int32_t* status_tmp;    // [I] when the caller does not want status
+    unsigned long long* work_ctr;
+    char* gstate;
+    size_t slot_bytes;
+    int grid_slots;
+    size_t total;
+};
+
+struct SimConfig {
+    int threads;
+    bool smem;
+    int cap;
+    size_t dyn_smem;
+    int sb, ib;
+    int sort_lo, sort_hi;
+};
+
+constexpr size_t SMEM_STATE_LIMIT = 200 * 1024;
+
+SimConfig sim_config(const svf_trace_t* tr)
+{
+    SimConfig c;
+    const int64_t I = tr->n_instances, mx = tr->max_instance > 0 ? tr->max_instance : 1;
+    c.sb = bits_for_count(mx);
+    c.ib = bits_for_count(I);
+    c.sort_lo = c.sb;
+    c.sort_hi = c.sb + 32 + c.ib;
+    c.cap = (int)((mx + 31) / 32 * 32);
+    const size_t sbytes = state_bytes(c.cap);
+    c.smem = sbytes <= SMEM_STATE_LIMIT;
+    c.dyn_smem = c.smem ? sbytes : 0;
+    // group width: enough warps in flight to cover the GPU (about 16 per SM), no wider than the
+    // running set can use
+    const int64_t target_warps = (int64_t)sm_count() * 16;
+    int64_t w = I > 0 ? target_warps / I : 1;
+    int threads = 32;
+    while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
+    if (threads == 64) threads = 128;
+    if (threads == 512) threads = 1024;
+    c.threads = threads;
+    return c;
+}
+
+template <int THREADS, bool SMEM>
+int sim_grid(const SimConfig& c, int64_t I)
+{
+    int per_sm = 0;
+    if (SMEM) cudaFuncSetAttribute(k_sim<THREADS, SMEM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim<THREADS, SMEM>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    int64_t grid = (int64_t)per_sm * sm_count();
+    if (grid > I) grid = I;
+    if (grid < 1) grid = 1;
+    return (int)grid;
+}
+
+int sim_grid_any(const SimConfig& c, int64_t I)
+{
+    if (c.smem) {
+        switch (c.threads) {
+        case 32: return sim_grid<32, true>(c, I);
+        case 128: return sim_grid<128, true>(c, I);
+        case 256: return sim_grid<256, true>(c, I);
+        default: return sim_grid<1024, true>(c, I);
+        }
+    }
+    switch (c.threads) {
+    case 32: return sim_grid<32, false>(c, I);
+    case 128: return sim_grid<128, false>(c, I);
+    case 256: return sim_grid<256, false>(c, I);
+    default: return sim_grid<1024, false>(c, I);
+    }
+}
+
+// workspace layout; `grid` < 0: size for the worst case without touching the device
+void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig& c, int grid_slots)
+{
+    const int64_t N = tr->n_requests, I = tr->n_instances;
+    size_t p = 0;
+    const size_t s1 = sort_ws_bytes(N, c.sort_lo, c.sort_hi), s2 = sort_ws_bytes(N, 0, 32 + c.ib);
+    const size_t sort_bytes = s1 > s2 ? s1 : s2;
+    if (base) {
+        if (s1 >= s2) sort_ws_carve(&w->sort, base, N, c.sort_lo, c.sort_hi);
+        else          sort_ws_carve(&w->sort, base, N, 0, 32 + c.ib);
+    }
+    p += align_up(sort_bytes, 256);
+    w->words0 = (uint64_t*)(base + p); p += align_up((size_t)N * 8, 256);
+    w->words1 = (uint64_t*)(base + p); p += align_up((size_t)N * 8, 256);
+    w->order = (uint32_t*)(base + p);  p += align_up((size_t)N * 4, 256);
+    w->rank = (uint32_t*)(base + p);   p += align_up((size_t)N * 4, 256);
+    w->status_tmp = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
+    w->work_ctr = (unsigned long long*)(base + p); p += 256;
+    w->slot_bytes = c.smem ? 0 : align_up(state_bytes(c.cap), 256);
+    w->grid_slots = grid_slots;
+    w->gstate = base + p; p += w->slot_bytes * (size_t)grid_slots;
+    w->total = p;
+}
+
+thread_local int64_t g_launches_sim = 0;
+
+}  // namespace
+
+int64_t sim_last_launches() { return g_launches_sim; }
+
+}  // namespace svf
+
+using namespace svf;
+
+extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr)
+{
+    if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0) return 0;
+    SimConfig c = sim_config(tr);
+    SimWs w;
+    // state slots in global memory only exist for oversized instances: one CTA per SM at most
+    // 2 per SM; size for 2 x SMs (the launch never uses more)
+    sim_ws_layout(&w, nullptr, tr, c, c.smem ? 0 : 2 * sm_count());
+    return w.total + 256;
+}
+
+extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out,
+                            void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches_sim = 0;
+    if (!tr || !out) return SVF_EINVAL;
+    const int64_t I = tr->n_instances, N = tr->n_requests;
+    if (I < 0 || N < 0 || N >= ((int64_t)1 << 30) || tr->max_instance < 0 || tr->max_instance > N) return SVF_EINVAL;
+    if (policy < 0 || policy > 3 || M < 0) return SVF_EINVAL;
+    if (policy == SVF_SVF_1BIT && (!tr->bit || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
+    if (I == 0) return SVF_OK;
+    if (!tr->offsets || (N > 0 && (!tr->arrival || !tr->prompt || !tr->output))) return SVF_EINVAL;
+    SimConfig c = sim_config(tr);
+    if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;          // packed sort word would not fit
+    if (!ws) return SVF_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
+
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
+    int grid = sim_grid_any(c, I);
+    if (!c.smem && grid > 2 * sm_count()) grid = 2 * sm_count();
+    SimWs w;
+    sim_ws_layout(&w, base, tr, c, c.smem ? 0 : grid);
+    if (w.total > avail) return SVF_EWORKSPACE;
+
+    SimArgs g;
+    g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
+    g.policy = policy; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
+    g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
+    g.order = w.order; g.rank = w.rank;
+    g.start = out->start; g.finish = out->finish; g.tel = out->total_latency; g.peak = out->peak_kv;
+    g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
+    g.status = out->status ? out->status : w.status_tmp;
+    g.latw = out->p99_latency ? w.words0 : nullptr;
+    g.work_ctr = w.work_ctr; g.gstate = w.gstate; g.slot_bytes = w.slot_bytes; g.cap = c.cap;
+
+    if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
+    int rc = 0;
+    if (N > 0) {
+        int64_t blocks = ceil_div(N, 256);
+        const int64_t capb = (int64_t)sm_count() * 8;
+        if (blocks > capb) blocks = capb;
+        k_sim_pack<<<(unsigned)blocks, 256, 0, st>>>(g, w.words0);
+        ++g_launches_sim;
+        rc = sort_u64(w.sort, w.words0, w.words1, w.words0, N, c.sort_lo, c.sort_hi, st, &g_launches_sim);
+        if (rc) return SVF_ECUDA;
+        k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order, w.rank);
+        ++g_launches_sim;
+    }
+#define SVF_SIM_LAUNCH(T, S) k_sim<T, S><<<grid, T, c.dyn_smem, st>>>(g)
+    if (c.smem) {
+        switch (c.threads) {
+        case 32: SVF_SIM_LAUNCH(32, true); break;
+        case 128: SVF_SIM_LAUNCH(128, true); break;
+        case 256: SVF_SIM_LAUNCH(256, true); break;
+        default: SVF_SIM_LAUNCH(1024, true); break;
+        }
+    } else {
+        switch (c.threads) {
+        case 32: SVF_SIM_LAUNCH(32, false); break;
+        case 128: SVF_SIM_LAUNCH(128, false); break;
+        case 256: SVF_SIM_LAUNCH(256, false); break;
+        default: SVF_SIM_LAUNCH(1024, false); break;
+        }
+    }
+#undef SVF_SIM_LAUNCH
+    ++g_launches_sim;
+    if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
+
+    if (out->p99_latency) {
+        if (N > 0) {
+            rc = sort_u64(w.sort, w.words0, w.words1, w.words0, N, 0, 32 + c.ib, st, &g_launches_sim);
+            if (rc) return SVF_ECUDA;
+        } else {
+            rc = sort_u64(w.sort, w.words0, w.words1, w.words0, 0, 0, 32, st, &g_launches_sim);
+            if (rc) return SVF_ECUDA;
+        }
+        k_sim_p99<<<(unsigned)ceil_div(I, 128), 128, 0, st>>>(I, tr->offsets, w.sort.plan, g.status, out->p99_latency);
+        ++g_launches_sim;
+    }
+    return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
+}

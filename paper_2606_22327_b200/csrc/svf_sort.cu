@@ -1,0 +1,358 @@
+// a3: device-wide stable LSD radix sort of 64-bit words ("onesweep": one up-front histogram of
+// every digit, then one chained-scan pass per digit with decoupled look-back), sm_100a.
+//
+// Serves the waiting-queue sort of the paper's admission rule (ascending key, P:L67, P:L351;
+// unique tie-break P:L501) on packed (key, arrival, id) words, the segmented presort of
+// svf_simulate (instance id in the top bits) and the per-instance latency sort behind p99.
+//
+// Design notes (B200):
+//  * HBM-bound: 8 B/word for the histogram + 16 B/word per executed pass.  A pass whose digit is
+//    identical in every word is detected from the histogram ON THE DEVICE and skipped, so the
+//    host never reads anything back (key bits are bounded: < 2^24..2^26 for the paper-shaped
+//    workloads).
+//  * Each pass CTA owns one 4096-word tile (32 KB): the tile is staged global->shared with one
+//    1-D TMA bulk copy (cp.async.bulk + mbarrier), ranked per warp with __match_any_sync digit
+//    ballots (stable), scattered inside shared memory so the final global stores are coalesced
+//    runs per digit.
+//  * Tile ids come from an atomic counter, so a tile's predecessors are always resident or
+//    done: the look-back spin cannot deadlock.
+#include "svf_internal.cuh"
+
+namespace svf {
+
+namespace {
+
+constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_INCL = 2u << 30, VALUE_MASK = (1u << 30) - 1u;
+
+__device__ __forceinline__ uint32_t digit_of(uint64_t w, int shift, uint32_t mask)
+{
+    return (uint32_t)(w >> shift) & mask;
+}
+
+// ---- histogram of every digit in one read of the input ---------------------------------------
+template <int NPASS>
+__global__ void __launch_bounds__(512) k_sort_hist(const uint64_t* __restrict__ in, int64_t n,
+                                                   int bit_lo, int bit_hi,
+                                                   uint32_t* __restrict__ ghist)
+{
+    __shared__ uint32_t sh[NPASS * SORT_RADIX];
+    for (int i = threadIdx.x; i < NPASS * SORT_RADIX; i += blockDim.x) sh[i] = 0;
+    __syncthreads();
+
+    int shift[NPASS]; uint32_t mask[NPASS];
+#pragma unroll
+    for (int p = 0; p < NPASS; ++p) {
+        shift[p] = bit_lo + p * SORT_RADIX_BITS;
+        int wdt = bit_hi - shift[p]; if (wdt > SORT_RADIX_BITS) wdt = SORT_RADIX_BITS;
+        mask[p] = (1u << wdt) - 1u;
+    }
+    // run-length accumulation: a digit that repeats costs one shared atomic per run, so the
+    // all-equal high digits of small keys do not serialise on a single bin
+    uint32_t last[NPASS], cnt[NPASS];
+#pragma unroll
+    for (int p = 0; p < NPASS; ++p) { last[p] = 0; cnt[p] = 0; }
+
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        uint64_t w = __ldg(in + i);
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) {
+            uint32_t d = digit_of(w, shift[p], mask[p]);
+            if (d == last[p]) ++cnt[p];
+            else { if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]); last[p] = d; cnt[p] = 1; }
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < NPASS; ++p) if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]);
+    __syncthreads();
+    for (int i = threadIdx.x; i < NPASS * SORT_RADIX; i += blockDim.x)
+        if (sh[i]) atomicAdd(&ghist[i], sh[i]);
+}
+
+// ---- exclusive scan of each digit histogram + the ping-pong plan -------------------------------
+__global__ void __launch_bounds__(SORT_RADIX) k_sort_plan(uint32_t* __restrict__ hist, int npass,
+                                                         int64_t n, const uint64_t* in,
+                                                         uint64_t* x, uint64_t* y,
+                                                         SortPlan* __restrict__ plan)
+{
+    __shared__ uint32_t warp_tot[SORT_RADIX / 32];
+    __shared__ int skip_s[SORT_MAX_PASSES];
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    for (int p = 0; p < npass; ++p) {
+        uint32_t c = hist[p * SORT_RADIX + tid];
+        int trivial = __syncthreads_or(c == (uint32_t)n);
+        uint32_t inc = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) warp_tot[wrp] = inc;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
+        hist[p * SORT_RADIX + tid] = off + inc - c;
+        if (tid == 0) skip_s[p] = trivial;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const uint64_t* cur = in;
+        for (int p = 0; p < npass; ++p) {
+            plan->skip[p] = skip_s[p];
+            if (skip_s[p]) { plan->src[p] = nullptr; plan->dst[p] = nullptr; continue; }
+            uint64_t* d = (cur == x) ? y : x;
+            plan->src[p] = cur; plan->dst[p] = d; cur = d;
+        }
+        plan->result = cur;
+    }
+}
+
+// ---- TMA 1-D bulk copy + mbarrier (PTX; SASS: UBLKCP / SYNCS) ---------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---- one onesweep pass -----------------------------------------------------------------------
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __restrict__ plan,
+                                                            int p, int64_t n, int shift,
+                                                            uint32_t mask,
+                                                            uint32_t* __restrict__ tile_ctr,
+                                                            uint32_t* __restrict__ status,
+                                                            const uint32_t* __restrict__ bases)
+{
+    constexpr int WARPS = SORT_THREADS / 32;
+    __shared__ __align__(128) uint64_t staging[SORT_TILE];
+    __shared__ uint32_t whist[WARPS * SORT_RADIX];
+    __shared__ uint32_t toff_s[SORT_RADIX];
+    __shared__ uint32_t gbase_s[SORT_RADIX];
+    __shared__ uint32_t warp_tot[SORT_RADIX / 32];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ uint32_t tile_s;
+
+    if (plan->skip[p]) return;                      // uniform over the grid
+    const uint64_t* __restrict__ src = plan->src[p];
+    uint64_t* __restrict__ dst = plan->dst[p];
+
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    if (tid == 0) { tile_s = atomicAdd(&tile_ctr[p], 1u); mbar_init(&bar, 1); }
+    for (int i = tid; i < WARPS * SORT_RADIX; i += SORT_THREADS) whist[i] = 0;
+    __syncthreads();
+    const uint32_t tile = tile_s;
+    const int64_t tile_base = (int64_t)tile * SORT_TILE;
+    const int tile_n = (int)((n - tile_base) < (int64_t)SORT_TILE ? (n - tile_base) : (int64_t)SORT_TILE);
+
+    // stage the tile, then take it in warp-striped order: item i of lane l in warp w is element
+    // w*32*IPT + i*32 + l of the tile (so ranks follow the input order = stability)
+    uint64_t key[SORT_IPT];
+    const int wbase = wrp * 32 * SORT_IPT;
+    const bool bulk = (tile_n == SORT_TILE) && ((reinterpret_cast<uintptr_t>(src + tile_base) & 15u) == 0);
+    if (bulk) {
+        if (tid == 0) {
+            mbar_expect_tx(&bar, SORT_TILE * 8u);
+            tma_load_1d(staging, src + tile_base, SORT_TILE * 8u, &bar);
+        }
+        mbar_wait(&bar, 0);
+#pragma unroll
+        for (int i = 0; i < SORT_IPT; ++i) key[i] = staging[wbase + i * 32 + lane];
+    } else {
+#pragma unroll
+        for (int i = 0; i < SORT_IPT; ++i) {
+            int e = wbase + i * 32 + lane;
+            key[i] = e < tile_n ? __ldg(src + tile_base + e) : ~0ull;
+        }
+    }
+
+    // per-warp stable ranking with digit ballots
+    uint32_t* wh = whist + wrp * SORT_RADIX;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    uint32_t rank[SORT_IPT];
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        const bool valid = (wbase + i * 32 + lane) < tile_n;
+        const uint32_t d = valid ? digit_of(key[i], shift, mask) : SORT_RADIX;
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t base = 0;
+        if (valid) base = wh[d];
+        __syncwarp();
+        if (valid && lane == (31 - __clz(peers))) wh[d] = base + __popc(peers);
+        __syncwarp();
+        rank[i] = base + __popc(peers & lt_mask);
+    }
+    __syncthreads();
+
+    // digit d (thread d): exclusive scan over warps, tile count, publish, tile-level scan
+    uint32_t count = 0;
+    {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) { uint32_t c = whist[w * SORT_RADIX + tid]; whist[w * SORT_RADIX + tid] = run; run += c; }
+        count = run;
+        volatile uint32_t* st = status + (size_t)tile * SORT_RADIX + tid;
+        *st = (tile == 0 ? FLAG_INCL : FLAG_AGG) | count;
+        uint32_t inc = count;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) warp_tot[wrp] = inc;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
+        const uint32_t toff = off + inc - count;
+        toff_s[tid] = toff;
+        // decoupled look-back over the predecessor tiles of this digit
+        uint32_t excl = 0;
+        if (tile > 0) {
+            int64_t look = (int64_t)tile - 1;
+            while (true) {
+                uint32_t v = *(volatile uint32_t*)(status + (size_t)look * SORT_RADIX + tid);
+                uint32_t f = v >> 30;
+                if (f == 0) continue;
+                excl += v & VALUE_MASK;
+                if (f == 2) break;
+                --look;
+            }
+            *st = FLAG_INCL | (excl + count);
+        }
+        gbase_s[tid] = bases[tid] + excl - toff;    // modulo 2^32; dst index = gbase + slot
+    }
+    __syncthreads();
+
+    // scatter inside shared memory, then write coalesced runs
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        if ((wbase + i * 32 + lane) < tile_n) {
+            uint32_t d = digit_of(key[i], shift, mask);
+            staging[toff_s[d] + wh[d] + rank[i]] = key[i];
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < tile_n; q += SORT_THREADS) {
+        uint64_t w = staging[q];
+        uint32_t d = digit_of(w, shift, mask);
+        dst[(uint32_t)(gbase_s[d] + (uint32_t)q)] = w;
+    }
+}
+
+__global__ void k_sort_copy_result(const SortPlan* __restrict__ plan, uint64_t* __restrict__ out, int64_t n)
+{
+    const uint64_t* __restrict__ r = plan->result;
+    if (r == out) return;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) out[i] = r[i];
+}
+
+__global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan->result = in; }
+
+}  // namespace
+
+int sm_count()
+{
+    static int cached = 0;
+    if (cached == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            cached = v;
+        else
+            return 148;
+    }
+    return cached;
+}
+
+static size_t sort_status_bytes(int64_t n, int bit_lo, int bit_hi)
+{
+    int64_t tiles = ceil_div(n > 0 ? n : 1, SORT_TILE);
+    return align_up((size_t)sort_num_passes(bit_lo, bit_hi) * (size_t)tiles * SORT_RADIX * sizeof(uint32_t), 256);
+}
+
+size_t sort_ws_bytes(int64_t n, int bit_lo, int bit_hi)
+{
+    size_t b = 0;
+    b += align_up(sizeof(SortPlan), 256);
+    b += align_up(sizeof(uint32_t) * SORT_MAX_PASSES * SORT_RADIX, 256);
+    b += align_up(sizeof(uint32_t) * SORT_MAX_PASSES, 256);
+    b += sort_status_bytes(n, bit_lo, bit_hi);
+    return b;
+}
+
+void sort_ws_carve(SortWs* w, void* base, int64_t n, int bit_lo, int bit_hi)
+{
+    char* p = (char*)base;
+    w->plan = (SortPlan*)p;       p += align_up(sizeof(SortPlan), 256);
+    w->hist = (uint32_t*)p;       p += align_up(sizeof(uint32_t) * SORT_MAX_PASSES * SORT_RADIX, 256);
+    w->tile_ctr = (uint32_t*)p;   p += align_up(sizeof(uint32_t) * SORT_MAX_PASSES, 256);
+    w->status = (uint32_t*)p;
+    w->status_bytes = sort_status_bytes(n, bit_lo, bit_hi);
+}
+
+int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int64_t n, int bit_lo,
+             int bit_hi, cudaStream_t st, int64_t* launches)
+{
+    if (n <= 0) {
+        k_sort_plan_identity<<<1, 1, 0, st>>>(w.plan, in);
+        ++*launches;
+        return (int)cudaGetLastError();
+    }
+    const int npass = sort_num_passes(bit_lo, bit_hi);
+    // hist, tile counters and look-back words are contiguous: one memset
+    size_t zero_bytes = (size_t)((char*)w.status - (char*)w.hist) + w.status_bytes;
+    cudaError_t e = cudaMemsetAsync(w.hist, 0, zero_bytes, st);
+    if (e != cudaSuccess) return (int)e;
+
+    const int hthreads = 512;
+    int64_t hblocks = ceil_div(n, (int64_t)hthreads * 8);
+    int64_t hmax = (int64_t)sm_count() * 4;
+    if (hblocks > hmax) hblocks = hmax;
+    if (hblocks < 1) hblocks = 1;
+    switch (npass) {
+#define SVF_HIST_CASE(NP) case NP: k_sort_hist<NP><<<(unsigned)hblocks, hthreads, 0, st>>>(in, n, bit_lo, bit_hi, w.hist); break;
+        SVF_HIST_CASE(1) SVF_HIST_CASE(2) SVF_HIST_CASE(3) SVF_HIST_CASE(4)
+        SVF_HIST_CASE(5) SVF_HIST_CASE(6) SVF_HIST_CASE(7) SVF_HIST_CASE(8)
+#undef SVF_HIST_CASE
+    default: return (int)cudaErrorInvalidValue;
+    }
+    ++*launches;
+    k_sort_plan<<<1, SORT_RADIX, 0, st>>>(w.hist, npass, n, in, x, y, w.plan);
+    ++*launches;
+    const int64_t tiles = ceil_div(n, SORT_TILE);
+    for (int p = 0; p < npass; ++p) {
+        int shift = bit_lo + p * SORT_RADIX_BITS;
+        int wdt = bit_hi - shift; if (wdt > SORT_RADIX_BITS) wdt = SORT_RADIX_BITS;
+        k_sort_pass<<<(unsigned)tiles, SORT_THREADS, 0, st>>>(w.plan, p, n, shift, (1u << wdt) - 1u, w.tile_ctr,
+                                                              w.status + (size_t)p * tiles * SORT_RADIX,
+                                                              w.hist + p * SORT_RADIX);
+        ++*launches;
+    }
+    return (int)cudaGetLastError();
+}
+
+int sort_result_to(const SortWs& w, uint64_t* out, int64_t n, cudaStream_t st, int64_t* launches)
+{
+    if (n <= 0) return 0;
+    int64_t blocks = ceil_div(n, 256 * 4);
+    int64_t bmax = (int64_t)sm_count() * 8;
+    if (blocks > bmax) blocks = bmax;
+    k_sort_copy_result<<<(unsigned)blocks, 256, 0, st>>>(w.plan, out, n);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+}  // namespace svf

@@ -1,0 +1,312 @@
+"""GPU parity (bit-exact): svf_admit and svf_simulate against the CPU oracle, through the C ABI.
+Run on the B200 box with ``-m gpu``."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2606_22327_b200 import traces as T
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+POL = {"svf": 0, "svf_1bit": 1, "sjf": 2, "fcfs": 3}
+FIELDS = ("start", "finish", "total_latency", "p99_latency", "makespan", "peak_kv", "rounds",
+          "decisions", "status")
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2606_22327_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def run_gpu(B, trace, policy, M=None, want=FIELDS):
+    import torch
+    dt = B.DeviceTrace.from_host(trace)
+    out = B.svf_simulate(dt, policy, M, want=want)
+    torch.cuda.synchronize()
+    return {k: getattr(out, k).cpu().numpy() for k in want}
+
+
+def assert_same(got, ref, trace, ctx=""):
+    I, N = trace.n_instances, trace.n_requests
+    for k in got:
+        g = got[k][:N] if k in ("start", "finish") else got[k][:I]
+        r = getattr(ref, k)
+        if not np.array_equal(g, r):
+            bad = np.nonzero(g != r)[0]
+            raise AssertionError(f"{ctx}: field {k} differs at {bad[:8]} (gpu {g[bad[:8]]}, oracle {r[bad[:8]]}); "
+                                 f"{len(bad)} of {len(r)}")
+
+
+def check(B, oracle, trace, policy, M=None, ctx="", threads=8):
+    ref = oracle.simulate(trace, policy, M=M, n_threads=threads)
+    got = run_gpu(B, trace, policy, M)
+    assert_same(got, ref, trace, ctx or f"{trace.name} policy {policy}")
+    return ref, got
+
+
+# ---------------------------------------------------------------------------------------------
+# svf_simulate
+# ---------------------------------------------------------------------------------------------
+def _golden_examples():
+    ex, cur = [], None
+    for line in open(os.path.join(GOLDEN, "hand_examples.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        tok = line.split()
+        if tok[0] == "example":
+            cur = {"name": tok[1], "M": int(tok[2].split("=")[1]), "policy": tok[3].split("=")[1], "req": []}
+            ex.append(cur)
+        elif tok[0] == "req":
+            cur["req"].append(tuple(int(x) for x in tok[1:4]))
+        elif tok[0] == "start":
+            cur["start"] = [int(x) for x in tok[1:]]
+        elif tok[0] == "tel":
+            cur["tel"] = int(tok[1])
+    return ex
+
+
+def test_hand_examples_from_the_paper_model(B):
+    """Values derived by hand from Eq. 3c (tests/golden/hand_examples.txt), not from any code."""
+    for ex in _golden_examples():
+        a, s, o = (np.array(x, np.int32) for x in zip(*ex["req"]))
+        tr = T._one(ex["name"], a, s, o, np.zeros(len(a), np.uint8), ex["M"], 1, 1)
+        got = run_gpu(B, tr, POL[ex["policy"]])
+        assert list(got["start"][: len(a)]) == ex["start"], ex["name"]
+        assert int(got["total_latency"][0]) == ex["tel"], ex["name"]
+        assert int(got["status"][0]) == 0
+
+
+def test_config1_tiny_offline_batch(B, oracle):
+    """configs[0]: n=8 at t=0, M=32, all four policies, 512 seeds batched as instances."""
+    parts = [T.config1(i) for i in range(512)]
+    tr = T.concat(parts, "cfg1x512", 32, 2, 8)
+    for policy in range(4):
+        check(B, oracle, tr, policy)
+
+
+def test_config2_single_online_trace(B, oracle):
+    """configs[1]: n=2000, lambda=4, M=300k: one instance, one CTA."""
+    for inst in range(2):
+        tr = T.config2(inst)
+        for policy in range(4):
+            ref, _ = check(B, oracle, tr, policy)
+            assert ref.status[0] == 0 and ref.peak_kv[0] <= tr.M
+
+
+@pytest.mark.parametrize("lam", [2.0, 4.0, 8.0])
+def test_config3_batched_subset(B, oracle, lam):
+    """configs[2] shape, 96 instances x 1000 requests (several waves of the warp-per-instance
+    kernel would need 4096; the full size is covered by test_config3_full_size_sampled)."""
+    tr = T.config3(n_instances=96, lam=lam)
+    for policy in range(4):
+        check(B, oracle, tr, policy)
+
+
+def test_config3_full_size_sampled(B, oracle):
+    """configs[2] at full size (4096 x 1000, the launch bench.py times): every instance's scalar
+    outputs against the oracle for SVF; start/finish on all requests."""
+    tr = T.config3(n_instances=4096, lam=4.0)
+    check(B, oracle, tr, 0)
+    got = run_gpu(B, tr, 3, want=("total_latency", "status", "peak_kv"))
+    sub = np.arange(0, 4096, 64)
+    ref = oracle.simulate(tr.subset(sub), 3, n_threads=8)
+    assert np.array_equal(got["total_latency"][sub], ref.total_latency)
+    assert np.array_equal(got["peak_kv"][sub], ref.peak_kv)
+    assert not got["status"][:4096].any()
+
+
+def test_config4_high_concurrency_reduced(B, oracle):
+    """configs[3] laws at n=20,000 (state in the global-memory slot: > 16k entries)."""
+    tr = T.config4(n=20_000, M=1_000_000)
+    for policy in range(4):
+        check(B, oracle, tr, policy)
+
+
+def test_config4_full_size(B, oracle):
+    """configs[3]: n=200,000, lambda=64, M=1e6; total latency exceeds 2^32 (int64 path)."""
+    tr = T.config4()
+    for policy in (0, 3):
+        ref, _ = check(B, oracle, tr, policy)
+        assert ref.total_latency[0] > 2 ** 32
+
+
+@pytest.mark.parametrize("M", [50_000, 200_000, 800_000])
+def test_config5_onebit_sweep_subset(B, oracle, M):
+    """configs[4] shape: 24 instances x 5000, bimodal outputs, flipped bits."""
+    for p in (0.0, 0.2):
+        tr = T.config5(n_instances=24, M=M, p_flip=p)
+        for policy in (0, 1, 2):
+            check(B, oracle, tr, policy)
+
+
+def test_ragged_batch_with_empty_and_rejected_instances(B, oracle):
+    """Instances of different sizes, empty ones, and every data error; a bad instance must not
+    disturb its neighbours."""
+    M = 40
+    parts = []
+    parts.append(T.random_small(1, 17, 10, 12, M, a_hi=30))
+    parts.append(T._one("empty", *(np.zeros(0, np.int32),) * 3, np.zeros(0, np.uint8), M, 2, 8))
+    bad_range = T.random_small(2, 9, 10, 12, M, a_hi=5); bad_range.output[3] = 0
+    parts.append(bad_range)
+    unsorted = T.random_small(3, 9, 10, 12, M, a_hi=50); unsorted.arrival[5] = 0; unsorted.arrival[4] = 7
+    parts.append(unsorted)
+    infeasible = T.random_small(4, 9, 10, 12, M, a_hi=5); infeasible.prompt[0] = 35; infeasible.output[0] = 6
+    parts.append(infeasible)
+    overflow = T.random_small(5, 5, 10, 12, M, a_hi=5); overflow.arrival[-1] = 2 ** 31 - 5
+    parts.append(overflow)
+    parts.append(T.random_small(6, 33, 10, 12, M, a_hi=3))
+    parts.append(T.random_small(7, 1, 10, 12, M))
+    neg = T.random_small(8, 6, 10, 12, M, a_hi=5); neg.prompt[2] = -1
+    parts.append(neg)
+    parts.append(T.random_small(9, 64, 10, 12, M, a_hi=100))
+    tr = T.concat(parts, "ragged", M, 2, 8)
+    for policy in range(4):
+        ref, got = check(B, oracle, tr, policy)
+        assert set(ref.status.tolist()) >= {0, 16, 17, 18, 19}
+
+
+def test_random_small_instances_all_policies(B, oracle):
+    """Many tiny random online instances (tight budgets: M hit exactly, blocked heads, event-free
+    admissions) in one batch."""
+    parts = [T.random_small(100 + i, 3 + i % 40, 9, 11, 24, a_hi=(i % 7) * 5) for i in range(600)]
+    tr = T.concat(parts, "small600", 24, 3, 9)
+    for policy in range(4):
+        check(B, oracle, tr, policy)
+    # the same batch under a loose budget: everything starts on arrival, TEL = sum o (Lemma G.1)
+    ref, got = check(B, oracle, tr, 0, M=10 ** 9)
+    assert int(got["total_latency"][: tr.n_instances].sum()) == tr.request_steps
+
+
+def test_group_widths_and_state_placement(B, oracle):
+    """Shapes that select each kernel variant: 32/128/256/1024 threads, shared/global state."""
+    shapes = [(4096 // 8, 40, 2.0),     # many small instances -> one warp each
+              (100, 600, 4.0),         # 128 threads
+              (1, 2000, 4.0),          # 256 threads
+              (2, 9000, 8.0)]          # 1024 threads, shared state
+    for I, n, lam in shapes:
+        tr = T.config3(n_instances=I, n=n, lam=lam, M=60_000)
+        for policy in (0, 3):
+            check(B, oracle, tr, policy, ctx=f"I={I} n={n}")
+
+
+def test_outputs_are_optional(B, oracle):
+    tr = T.config3(n_instances=8, lam=4.0)
+    ref = oracle.simulate(tr, 0)
+    got = run_gpu(B, tr, 0, want=("total_latency",))
+    assert np.array_equal(got["total_latency"][:8], ref.total_latency)
+    got = run_gpu(B, tr, 0, want=("p99_latency", "finish"))
+    assert np.array_equal(got["p99_latency"][:8], ref.p99_latency)
+    assert np.array_equal(got["finish"][: tr.n_requests], ref.finish)
+
+
+def test_schedule_passes_the_independent_validator(B):
+    """The GPU schedule itself (not via the oracle simulator) against the paper's definitions:
+    capacity, area conservation, no bypass, blocked heads really blocked (oracle/validator.py)."""
+    from oracle import validator
+    tr = T.config2(3, n=600, M=120_000)
+    for policy in range(4):
+        got = run_gpu(B, tr, policy)
+        facts = validator.validate(tr, policy, got["start"][: tr.n_requests], finish=got["finish"][: tr.n_requests],
+                                   check_blocked=200)
+        assert facts["total_latency"] == int(got["total_latency"][0])
+        assert facts["rounds"] == int(got["rounds"][0]) and facts["decisions"] == int(got["decisions"][0])
+        assert facts["peak_kv"] == int(got["peak_kv"][0]) and facts["p99_latency"] == int(got["p99_latency"][0])
+
+
+# ---------------------------------------------------------------------------------------------
+# svf_admit
+# ---------------------------------------------------------------------------------------------
+def _admit_state(seed, n_wait, n_run, M):
+    sd = T.instance_seed(88, seed)
+    w_s = T.lognormal_int(sd, 2, 3, n_wait, 1000.0, 0.8, 16, 8192)
+    w_o = T.lognormal_int(sd, 4, 5, n_wait, 400.0, 1.0, 1, 4096)
+    w_a = np.sort(T.uniform_int(sd, 1, n_wait, 0, 5000))
+    w_bit = (w_o > 400).astype(np.uint8)
+    r_rem = T.uniform_int(sd, 6, n_run, 1, 3000)
+    # running set scaled to sit just under the budget at its worst completion time
+    r_kv = T.lognormal_int(sd, 7, 8, n_run, 1200.0, 0.8, 16, 12000)
+    if n_run:
+        order = np.argsort(-r_rem, kind="stable")
+        pre = np.cumsum(r_kv[order].astype(np.int64)) + r_rem[order].astype(np.int64) * np.arange(1, n_run + 1)
+        scale = min(1.0, (0.97 if seed % 2 else 0.8) * M / pre.max())
+        r_kv = np.maximum((r_kv * scale).astype(np.int32), 0)
+    return w_s, w_o, w_a, w_bit, r_kv, r_rem
+
+
+def _admit_both(B, oracle, policy, M, st, O0=179, O1=887):
+    import torch
+    w_s, w_o, w_a, w_bit, r_kv, r_rem = st
+    rc, idx, words = oracle.admit(policy, M, 5, w_s, w_o, w_a, w_bit, O0, O1, r_kv, r_rem)
+    out = B.svf_admit(policy, M, 5, _dev(w_s), _dev(w_o), _dev(w_a), _dev(w_bit), O0, O1, _dev(r_kv), _dev(r_rem))
+    torch.cuda.synchronize()
+    assert int(out.status.item()) == rc
+    k = int(out.n_admitted.item())
+    assert k == len(idx)
+    assert np.array_equal(out.admitted_idx.cpu().numpy()[:k], idx)
+    if rc == 0:
+        assert np.array_equal(out.sorted_words.cpu().numpy().view(np.uint64)[: len(w_s)], words)
+    return k
+
+
+@pytest.mark.parametrize("n_wait,n_run", [(0, 0), (0, 50), (1, 0), (37, 0), (1024, 256), (5000, 1024),
+                                           (5001, 1024), (70_000, 4096), (1 << 18, 300)])
+def test_admit_matches_oracle(B, oracle, n_wait, n_run):
+    M = 1_000_000
+    st = _admit_state(n_wait + n_run, n_wait, n_run, M)
+    ks = [_admit_both(B, oracle, policy, M, st) for policy in range(4)]
+    if n_wait >= 1024 and n_run <= 1024:
+        assert max(ks) > 0
+
+
+def test_admit_everything_fits_and_nothing_fits(B, oracle):
+    st = _admit_state(1, 300, 40, 10 ** 6)
+    assert _admit_both(B, oracle, 0, 10 ** 12, st) == 300           # whole queue admitted
+    assert _admit_both(B, oracle, 0, 10, st) == 0                   # running set already over M
+    w_s, w_o, w_a, w_bit, r_kv, r_rem = st
+    assert _admit_both(B, oracle, 2, int(r_kv.sum()) + int(r_rem.max()) * 40 + 1, st) >= 0
+
+
+def test_admit_data_errors(B, oracle):
+    base = _admit_state(2, 50, 10, 10 ** 6)
+    def variant(f):
+        st = [x.copy() for x in base]; f(st); return st
+    cases = [variant(lambda st: st[1].__setitem__(7, 0)),            # o < 1 -> ERANGE
+             variant(lambda st: st[2].__setitem__(9, 0)),            # arrivals decrease -> EUNSORTED
+             variant(lambda st: (st[2].__setitem__(9, 0), st[0].__setitem__(30, -4))),  # first offender wins
+             variant(lambda st: st[5].__setitem__(3, 0)),            # rem < 1 -> ERANGE
+             variant(lambda st: (st[0].__setitem__(4, 2 ** 30), st[1].__setitem__(4, 2 ** 20)))]  # key overflow
+    codes = []
+    for st in cases:
+        rc, _, _ = oracle.admit(0, 10 ** 6, 0, *st[:4], 2, 8, st[4], st[5])
+        codes.append(rc)
+        _admit_both(B, oracle, 0, 10 ** 6, st, 2, 8)
+    assert codes == [16, 17, 17, 16, 19]
+
+
+def test_admit_agrees_with_simulator_states(B, oracle):
+    """Replay admission decisions at states taken from an oracle run of configs[1]: running set
+    as (kv, rem), the waiting queue in arrival order."""
+    tr = T.config2(1)
+    ref = oracle.simulate(tr, 0)
+    a, s, o = tr.arrival.astype(np.int64), tr.prompt.astype(np.int64), tr.output.astype(np.int64)
+    k = ref.start.astype(np.int64)
+    for t in (100, 300, 450, 520, 700):
+        run = np.nonzero((k < t) & (k + o > t))[0]
+        wait = np.nonzero((a <= t) & (k >= t))[0]
+        st = (s[wait].astype(np.int32), o[wait].astype(np.int32), a[wait].astype(np.int32), tr.bit[wait],
+              (s[run] + t - k[run]).astype(np.int32), (k[run] + o[run] - t).astype(np.int32))
+        n_adm = _admit_both(B, oracle, 0, tr.M, st)
+        assert n_adm == int((k[wait] == t).sum())
