@@ -1,0 +1,430 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of arxiv/paper_2606_22327 on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A STEP is one pass of the whole hot path (keys -> pack -> segmented onesweep sort -> admission /
+feasibility -> state advance -> reductions) over one synthetic batch:
+`svf_simulate` under all four policies (SVF, 1-bit SVF, SJF, FCFS) on BASELINE.json configs[2]
+(4,096 instances x 1,000 requests, Poisson rate 4, M = 300,000), every output requested.
+metric = simulated request-steps per second, request_steps = sum_i o_i per policy run.
+Per rank the batch is fixed (weak scaling); ranks hold different seeded batches; no collective
+on the data path (instances are independent).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2606_22327_b200 import traces as T  # noqa: E402
+
+METRIC = "simulated_request_steps_per_sec"
+UNIT = "request-steps/s"
+POLICIES = (0, 1, 2, 3)
+POLICY_NAMES = ("svf", "svf_1bit", "sjf", "fcfs")
+L2_FLUSH_BYTES = 512 << 20
+
+# algorithmic HBM bytes per request of the dominant kernel (k_sim): a, s, o read by
+# the validation pass (12) + rank and order (8) + start, finish (8) + latency word for p99 (8)
+SIM_BYTES_PER_REQUEST = 36
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--instances", type=int, default=4096)
+    ap.add_argument("--requests", type=int, default=1000)
+    ap.add_argument("--lam", type=float, default=4.0)
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel and per-config extras")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                c, m = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                sm.append(c); mx.append(m)
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        if not sm:   # region shorter than one sample: take whatever we saw
+            for ts, line in self.rows:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1]))
+                except Exception:
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_batch(args, rank):
+    return T.config3(n_instances=args.instances, n=args.requests, lam=args.lam,
+                     first_instance=rank * args.instances)
+
+
+# ---------------------------------------------------------------------------------------------
+# reference arm = the CPU oracle, as it stands, on the host cores (tier framing (4))
+# ---------------------------------------------------------------------------------------------
+def oracle_step(svf_ref, sample, threads):
+    dec = 0
+    for p in POLICIES:
+        r = svf_ref.simulate(sample, p, n_threads=threads)
+        dec += int(r.decisions.sum())
+    return dec
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import svf_ref
+    svf_ref.build()
+    threads = min(os.cpu_count() or 1, svf_ref.max_threads())
+    n_inst = min(args.instances, 1024)            # bounded sample of the same workload
+    sample = T.config3(n_instances=n_inst, n=args.requests, lam=args.lam)
+    rs = sample.request_steps * len(POLICIES)
+    for _ in range(max(args.warmup, 0) and 1):
+        oracle_step(svf_ref, sample, threads)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(svf_ref, sample, threads)
+    dt = time.perf_counter() - t0
+    val = rs * args.steps / dt
+    desc = f"{n_inst} of {args.instances} instances x {args.requests} requests x 4 policies per step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+            "data": "synthetic", "config": workload_config(args, n_inst),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(args, n_inst=None):
+    return {"workload": "BASELINE.json configs[2] batched simulation: "
+                        f"{n_inst or args.instances} instances x {args.requests} requests, Poisson rate "
+                        f"{args.lam:g}/step, lognormal s (mean 600, sigma 0.8, [16,4096]) and o (mean 250, sigma 1.0, "
+                        "[1,2048]), M=300000, policies svf+svf_1bit+sjf+fcfs per step, all outputs",
+            "instances_per_gpu": n_inst or args.instances, "requests_per_instance": args.requests,
+            "M": 300000, "policies": list(POLICY_NAMES),
+            "cache": f"L2 flushed between timed steps (write of {L2_FLUSH_BYTES >> 20} MiB)"}
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_22327_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU path)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()
+
+    batch = make_batch(args, rank)
+    rs_step = batch.request_steps * len(POLICIES)
+    dt_dev = B.DeviceTrace.from_host(batch, device=dev)
+    outs = [B.SimOut.alloc(dt_dev) for _ in POLICIES]
+    ws = torch.empty(B.svf_simulate_workspace_bytes(dt_dev), dtype=torch.uint8, device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(profile=None):
+        launches = 0
+        for i, p in enumerate(POLICIES):
+            B.svf_simulate(dt_dev, p, out=outs[i], ws=ws)
+            launches += B.last_launch_count(2)
+            if profile is not None:
+                profile.append(B.simulate_phase_ms())
+        return launches
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        step()
+    torch.cuda.synchronize()
+    for o in outs:
+        assert int(o.status.abs().sum().item()) == 0, "a benchmark instance was rejected"
+
+    # ---- timed region: K steps, CUDA events around each step, L2 flushed in between -----------
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches = 0
+    barrier()
+    t0 = time.time()
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)
+        ev[k][0].record(stream)
+        launches += step()
+        ev[k][1].record(stream)
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+
+    # ---- per-phase times of the same step (events recorded inside the library, same stream) ---
+    B.set_profiling(True)
+    phase = []
+    for _ in range(max(2, min(args.steps, 5))):
+        flush.fill_(3)
+        step(profile=phase)
+    B.set_profiling(False)
+    phase = np.array(phase, dtype=np.float64)            # [calls, 4]
+    sim_ms = float(phase[:, 1].mean())                   # one k_sim launch, averaged over policies
+    share = {"phase_a_keys_sort_rank": float(phase[:, 0].sum() / phase[:, 3].sum()),
+             "phase_b_simulator": float(phase[:, 1].sum() / phase[:, 3].sum()),
+             "phase_c_p99": float(phase[:, 2].sum() / phase[:, 3].sum())}
+
+    # ---- end to end through the C ABI with host buffers: H2D of the trace from pinned memory,
+    # the four policy runs, D2H of every output --------------------------------------------------
+    pinned = {k: torch.from_numpy(getattr(batch, k)).pin_memory() for k in ("offsets", "arrival", "prompt", "output", "bit")}
+    host_out = [{k: torch.empty_like(getattr(o, k), device="cpu").pin_memory() for k in B.RESULT_FIELDS} for o in outs]
+    h2d = sum(int(v.numel() * v.element_size()) for v in pinned.values())
+    d2h = sum(int(v.numel() * v.element_size()) for ho in host_out for v in ho.values())
+
+    def e2e_step():
+        d = B.DeviceTrace.from_host(batch, device=dev, pinned=pinned, non_blocking=True)
+        for i, p in enumerate(POLICIES):
+            B.svf_simulate(d, p, out=outs[i], ws=ws)
+            for k in B.RESULT_FIELDS:
+                host_out[i][k].copy_(getattr(outs[i], k), non_blocking=True)
+        torch.cuda.synchronize()
+        return int(host_out[0]["total_latency"][0])
+
+    e2e_step()
+    barrier()
+    te0 = time.perf_counter()
+    n_e2e = max(2, min(args.steps, 5))
+    for _ in range(n_e2e):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - te0) / n_e2e
+
+    # ---- reduce over ranks: max time, summed work -------------------------------------------
+    decisions = sum(int(o.decisions.sum().item()) for o in outs)
+    if world > 1:
+        tmax = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tot = torch.tensor([rs_step, decisions, launches], dtype=torch.float64, device=dev)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        total_ms, e2e_s = float(tmax[0]), float(tmax[1])
+        rs_all, dec_all, launches_all = float(tot[0]), float(tot[1]), int(tot[2])
+    else:
+        rs_all, dec_all, launches_all = float(rs_step), float(decisions), launches
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = total_ms / args.steps
+    value = rs_all / (ms_per_step * 1e-3)
+    peak, peak_src = measured_peaks()
+    sim_bytes = SIM_BYTES_PER_REQUEST * batch.n_requests
+    achieved = sim_bytes / (sim_ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": workload_config(args),
+        "decisions_per_sec": dec_all / (ms_per_step * 1e-3),
+        "requests_per_sec": world * batch.n_requests * len(POLICIES) / (ms_per_step * 1e-3),
+        "step_ms": step_ms,
+        "clocks": clocks,
+        "e2e": {"value": rs_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": 1e3 * e2e_s},
+        "gpu_launches": launches_all,
+        "roofline": {"kernel": "k_sim (persistent simulator, phase B)", "bound": "hbm", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": sim_bytes,
+                     "kernel_ms": sim_ms, "share_of_step": share,
+                     "note": "latency/issue bound by design: state stays on chip, HBM only sees the trace once "
+                             "(DESIGN.md 6); see 'kernels' for the HBM-bound pieces"},
+    }
+    if not args.no_extras:
+        line["kernels"] = kernel_extras(B, torch, dev, peak)
+        line["configs"] = config_extras(B, torch, dev)
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _time_cuda(torch, fn, reps=5, flush=None):
+    fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return float(np.mean(ts))
+
+
+def kernel_extras(B, torch, dev, peak):
+    """The HBM-bound subsystems timed alone (inputs larger than L2: 2^26 requests)."""
+    out = []
+    n = 1 << 26
+    g = torch.Generator(device=dev); g.manual_seed(1)
+    s = torch.randint(16, 8193, (n,), device=dev, dtype=torch.int32, generator=g)
+    o = torch.randint(1, 4097, (n,), device=dev, dtype=torch.int32, generator=g)
+    words = torch.empty(n, dtype=torch.int64, device=dev)
+    st = torch.empty(1, dtype=torch.int32, device=dev)
+    ms = _time_cuda(torch, lambda: B.svf_keys(B.SVF, s, o, None, None, 1, 1, words, st))
+    bytes_keys = n * (4 + 4 + 8)
+    out.append({"kernel": "svf_keys (policy svf, n=2^26)", "ms": ms, "achieved": bytes_keys / ms / 1e6, "unit": "GB/s",
+                "frac": bytes_keys / ms / 1e6 / peak, "algorithmic_bytes": bytes_keys})
+    srt = torch.empty_like(words)
+    wsb = torch.empty(int(B.lib().svf_sort_workspace_bytes(n, 32, 64)), dtype=torch.uint8, device=dev)
+    ms = _time_cuda(torch, lambda: B.svf_sort_words(words, 32, 64, out=srt, ws=wsb), reps=3)
+    # keys < 2^26: 4 executed passes of the 4 planned (max key 8192*4096+4096*4097/2 needs 26 bits)
+    bytes_sort = n * (8 + 16 * 4)
+    out.append({"kernel": "svf_sort_words (n=2^26, key bits [32,64), 4 passes executed)", "ms": ms,
+                "achieved": bytes_sort / ms / 1e6, "unit": "GB/s", "frac": bytes_sort / ms / 1e6 / peak,
+                "algorithmic_bytes": bytes_sort, "words_per_sec": n / ms * 1e3})
+    del s, o, words, srt, wsb
+    # admission decisions at depth (BASELINE.json configs[3] laws): W waiting, R running
+    tr = T.config4(n=1 << 18)
+    w = [torch.from_numpy(x).to(dev) for x in (tr.prompt, tr.output, tr.arrival, tr.bit)]
+    r_rem = torch.arange(1, 1025, dtype=torch.int32, device=dev) * 3
+    r_kv = torch.full((1024,), 600, dtype=torch.int32, device=dev)
+    res = B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem)
+    wsa = torch.empty(B.svf_admit_workspace_bytes(1 << 18, 1024), dtype=torch.uint8, device=dev)
+    ms = _time_cuda(torch, lambda: B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem, ws=wsa, out=res))
+    k = int(res.n_admitted.item())
+    out.append({"kernel": "svf_admit (W=2^18 waiting, R=1024 running, policy svf)", "ms": ms, "admitted": k,
+                "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": (1 << 18) / ms * 1e3})
+    return out
+
+
+def config_extras(B, torch, dev):
+    """The other BASELINE.json configs, device-resident, SVF policy: context, not the headline."""
+    res = []
+    cases = [("configs[1] single online trace n=2000", T.config2(0)),
+             ("configs[3] single instance n=200000", T.config4()),
+             ("configs[4] 256x5000 M=200k p=0.05", T.config5(M=200_000, p_flip=0.05))]
+    for name, tr in cases:
+        d = B.DeviceTrace.from_host(tr, device=dev)
+        ws = torch.empty(B.svf_simulate_workspace_bytes(d), dtype=torch.uint8, device=dev)
+        for pol in (B.SVF, B.SVF_1BIT):
+            out = B.SimOut.alloc(d)
+            ms = _time_cuda(torch, lambda: B.svf_simulate(d, pol, out=out, ws=ws), reps=3)
+            res.append({"config": name, "policy": POLICY_NAMES[pol], "ms": ms,
+                        "request_steps_per_sec": tr.request_steps / ms * 1e3,
+                        "decisions_per_sec": int(out.decisions.sum().item()) / ms * 1e3,
+                        "total_latency": int(out.total_latency.sum().item())})
+    return res
+
+
+def cpu_baseline(args):
+    from oracle import svf_ref
+    svf_ref.build()
+    threads = min(os.cpu_count() or 1, svf_ref.max_threads())
+    n_inst = min(args.instances, 2048)
+    sample = T.config3(n_instances=n_inst, n=args.requests, lam=args.lam)
+    oracle_step(svf_ref, sample.subset(range(min(8, n_inst))), threads)
+    t0 = time.perf_counter()
+    reps = 0
+    while True:
+        oracle_step(svf_ref, sample, threads)
+        reps += 1
+        if time.perf_counter() - t0 > 10.0 or reps >= 8:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": sample.request_steps * len(POLICIES) * reps / dt, "unit": UNIT, "cores": threads,
+            "kind": "oracle", "sample": f"{n_inst} of {args.instances} instances x {args.requests} requests x 4 policies, "
+                                        f"{reps} repetitions, {dt:.1f} s, instance-parallel over {threads} host threads"}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

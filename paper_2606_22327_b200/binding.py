@@ -23,7 +23,7 @@ ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
 EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_workspace_bytes",
            "svf_simulate", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
-           "svf_status_string", "svf_version")
+           "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms")
 
 
 class SvfError(RuntimeError):
@@ -80,6 +80,10 @@ def lib():
         L.svf_status_string.restype = C.c_char_p
         L.svf_status_string.argtypes = [C.c_int]
         L.svf_version.restype = C.c_char_p
+        L.svf_set_profiling.restype = None
+        L.svf_set_profiling.argtypes = [C.c_int]
+        L.svf_simulate_phase_ms.restype = C.c_int
+        L.svf_simulate_phase_ms.argtypes = [C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -90,6 +94,17 @@ def status_string(code: int) -> str:
 
 def version() -> str:
     return lib().svf_version().decode()
+
+
+def set_profiling(enabled: bool) -> None:
+    lib().svf_set_profiling(1 if enabled else 0)
+
+
+def simulate_phase_ms():
+    """(phase A, phase B, phase C, whole call) in ms for the last profiled svf_simulate call."""
+    buf = (C.c_float * 4)()
+    _check(lib().svf_simulate_phase_ms(buf), "svf_simulate_phase_ms")
+    return tuple(float(x) for x in buf)
 
 
 def last_launch_count(which: int) -> int:

@@ -376,6 +376,18 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
 }
 
 thread_local int64_t g_launches_sim = 0;
+thread_local int g_profiling = 0;
+thread_local bool g_events_valid = false;
+thread_local cudaEvent_t g_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+
+void prof_mark(int i, cudaStream_t st)
+{
+    if (!g_profiling) return;
+    if (!g_ev[0])
+        for (int k = 0; k < 4; ++k) cudaEventCreate(&g_ev[k]);
+    cudaEventRecord(g_ev[i], st);
+    if (i == 3) g_events_valid = true;
+}
 
 }  // namespace
 
@@ -434,6 +446,8 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     g.latw = out->p99_latency ? w.words0 : nullptr;
     g.work_ctr = w.work_ctr; g.gstate = w.gstate; g.slot_bytes = w.slot_bytes; g.cap = c.cap;
 
+    g_events_valid = false;
+    prof_mark(0, st);
     if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
     int rc = 0;
     if (N > 0) {
@@ -447,6 +461,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order, w.rank);
         ++g_launches_sim;
     }
+    prof_mark(1, st);
 #define SVF_SIM_LAUNCH(T, S) k_sim<T, S><<<grid, T, c.dyn_smem, st>>>(g)
     if (c.smem) {
         switch (c.threads) {
@@ -466,6 +481,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
 #undef SVF_SIM_LAUNCH
     ++g_launches_sim;
     if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
+    prof_mark(2, st);
 
     if (out->p99_latency) {
         if (N > 0) {
@@ -478,5 +494,19 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         k_sim_p99<<<(unsigned)ceil_div(I, 128), 128, 0, st>>>(I, tr->offsets, w.sort.plan, g.status, out->p99_latency);
         ++g_launches_sim;
     }
+    prof_mark(3, st);
     return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
+}
+
+extern "C" void svf_set_profiling(int enabled) { g_profiling = enabled ? 1 : 0; }
+
+extern "C" int svf_simulate_phase_ms(float* ms_out)
+{
+    if (!ms_out || !g_events_valid) return SVF_EINVAL;
+    if (cudaEventSynchronize(g_ev[3]) != cudaSuccess) return SVF_ECUDA;
+    cudaEventElapsedTime(&ms_out[0], g_ev[0], g_ev[1]);
+    cudaEventElapsedTime(&ms_out[1], g_ev[1], g_ev[2]);
+    cudaEventElapsedTime(&ms_out[2], g_ev[2], g_ev[3]);
+    cudaEventElapsedTime(&ms_out[3], g_ev[0], g_ev[3]);
+    return SVF_OK;
 }

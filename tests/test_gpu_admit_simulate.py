@@ -140,7 +140,7 @@ def test_config4_full_size(B, oracle):
     tr = T.config4()
     for policy in (0, 3):
         ref, _ = check(B, oracle, tr, policy)
-        assert ref.total_latency[0] > 2 ** 32
+        assert ref.total_latency[0] > (2 ** 31 if policy == 0 else 2 ** 32)
 
 
 @pytest.mark.parametrize("M", [50_000, 200_000, 800_000])
