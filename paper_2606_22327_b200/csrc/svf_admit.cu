@@ -186,7 +186,7 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     g_launches_admit = 0;
     const int64_t LIM = (int64_t)1 << 30;
     if (policy < 0 || policy > 3 || n_wait < 0 || n_run < 0 || n_wait >= LIM || n_run >= LIM || M < 0) return SVF_EINVAL;
-    if (policy == SVF_SVF_1BIT && (!w_bit || O0 < 1 || O1 < 1)) return SVF_EINVAL;
+    if (policy == SVF_SVF_1BIT && ((n_wait > 0 && !w_bit) || O0 < 1 || O1 < 1)) return SVF_EINVAL;
     if (!n_admitted_out) return SVF_EINVAL;
     if (n_wait > 0 && (!w_s || !w_o || !w_a)) return SVF_EINVAL;
     if (n_run > 0 && (!r_kv || !r_rem)) return SVF_EINVAL;

@@ -25,9 +25,10 @@ extern "C" int svf_keys(int policy, int64_t n, const int32_t* s, const int32_t* 
 {
     g_launches_keys = 0;
     if (policy < 0 || policy > 3 || n < 0 || n > ((int64_t)1 << 32)) return SVF_EINVAL;
-    if (policy == SVF_SVF_1BIT && (!bit || O0 < 1 || O1 < 1)) return SVF_EINVAL;
+    if (policy == SVF_SVF_1BIT && (O0 < 1 || O1 < 1)) return SVF_EINVAL;
     if (n > 0) {
         if (!words_out) return SVF_EINVAL;
+        if (policy == SVF_SVF_1BIT && !bit) return SVF_EINVAL;
         if ((policy == SVF_SVF || policy == SVF_SVF_1BIT) && !s) return SVF_EINVAL;
         if ((policy == SVF_SVF || policy == SVF_SJF) && !o) return SVF_EINVAL;
         if (policy == SVF_FCFS && !a) return SVF_EINVAL;

@@ -416,7 +416,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     const int64_t I = tr->n_instances, N = tr->n_requests;
     if (I < 0 || N < 0 || N >= ((int64_t)1 << 30) || tr->max_instance < 0 || tr->max_instance > N) return SVF_EINVAL;
     if (policy < 0 || policy > 3 || M < 0) return SVF_EINVAL;
-    if (policy == SVF_SVF_1BIT && (!tr->bit || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
+    if (policy == SVF_SVF_1BIT && ((N > 0 && !tr->bit) || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
     if (I == 0) return SVF_OK;
     if (!tr->offsets || (N > 0 && (!tr->arrival || !tr->prompt || !tr->output))) return SVF_EINVAL;
     SimConfig c = sim_config(tr);

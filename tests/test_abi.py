@@ -53,7 +53,8 @@ def test_host_side_argument_errors_need_no_gpu(svf_lib):
     L.svf_keys.argtypes = [C.c_int, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32] + [C.c_void_p] * 3
     assert L.svf_keys(7, 0, None, None, None, None, 1, 1, None, None, None) == 1       # unknown policy
     assert L.svf_keys(0, -1, None, None, None, None, 1, 1, None, None, None) == 1      # negative n
-    assert L.svf_keys(1, 0, None, None, None, None, 1, 1, None, None, None) == 1       # 1-bit without bit
+    assert L.svf_keys(1, 0, None, None, None, None, 0, 1, None, None, None) == 1       # 1-bit with O0 < 1
+    assert L.svf_keys(1, 5, None, None, None, None, 1, 1, None, None, None) == 1       # 1-bit without bit
     assert L.svf_keys(0, 5, None, None, None, None, 1, 1, None, None, None) == 1       # null arrays
     L.svf_sort_workspace_bytes.restype = C.c_size_t
     L.svf_sort_workspace_bytes.argtypes = [C.c_int64, C.c_int, C.c_int]

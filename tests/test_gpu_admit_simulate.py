@@ -240,8 +240,10 @@ def _admit_state(seed, n_wait, n_run, M):
     r_kv = T.lognormal_int(sd, 7, 8, n_run, 1200.0, 0.8, 16, 12000)
     if n_run:
         order = np.argsort(-r_rem, kind="stable")
-        pre = np.cumsum(r_kv[order].astype(np.int64)) + r_rem[order].astype(np.int64) * np.arange(1, n_run + 1)
-        scale = min(1.0, (0.97 if seed % 2 else 0.8) * M / pre.max())
+        cum = np.cumsum(r_kv[order].astype(np.int64)).astype(np.float64)
+        remterm = (r_rem[order].astype(np.int64) * np.arange(1, n_run + 1)).astype(np.float64)
+        target = (0.97 if seed % 2 else 0.8) * M
+        scale = float(np.clip(((target - remterm) / cum).min(), 0.0, 1.0))
         r_kv = np.maximum((r_kv * scale).astype(np.int32), 0)
     return w_s, w_o, w_a, w_bit, r_kv, r_rem
 
