@@ -138,13 +138,20 @@ int svf_sort_words(int64_t n, const uint64_t* words_in, uint64_t* words_out, int
  * 3 = svf_sort_words. */
 int64_t svf_last_launch_count(int which);
 
-/* Measurement aid.  svf_set_profiling(1): later svf_simulate calls on this host thread record
+/* Measurement aids.  svf_set_profiling(1): later svf_simulate calls on this host thread record
  * CUDA events on their stream around the three phases.  svf_simulate_phase_ms waits for the
  * events of the last such call and writes ms_out ([host] float[4]): [0] phase A (keys + pack +
  * segmented sort + rank), [1] phase B (the persistent simulator kernel), [2] phase C (p99 sort +
- * gather; 0 if not requested), [3] the whole call.  Returns SVF_EINVAL if profiling was off. */
-void svf_set_profiling(int enabled);
+ * gather; 0 if not requested), [3] the whole call.  Returns SVF_EINVAL if profiling was off.
+ * svf_set_profiling(2): as 1, and the simulator kernel also counts its algorithmic work (a
+ * slower variant of the same kernel, same results; M < 2^30 only): svf_simulate_work_counts
+ * synchronises and writes counts_out ([host] uint64[2]): [0] E = running entries examined,
+ * summed over every head evaluation (a4), [1] U = running entries updated, summed over every
+ * admission (a5).  The counts live in the workspace of that call, which must still be
+ * allocated.  svf_set_profiling(0) switches both off. */
+void svf_set_profiling(int mode);
 int svf_simulate_phase_ms(float* ms_out);
+int svf_simulate_work_counts(uint64_t* counts_out);
 
 const char* svf_status_string(int status);
 const char* svf_version(void);

@@ -23,7 +23,8 @@ ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
 EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_workspace_bytes",
            "svf_simulate", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
-           "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms")
+           "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
+           "svf_simulate_work_counts")
 
 
 class SvfError(RuntimeError):
@@ -84,6 +85,8 @@ def lib():
         L.svf_set_profiling.argtypes = [C.c_int]
         L.svf_simulate_phase_ms.restype = C.c_int
         L.svf_simulate_phase_ms.argtypes = [C.POINTER(C.c_float)]
+        L.svf_simulate_work_counts.restype = C.c_int
+        L.svf_simulate_work_counts.argtypes = [C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
 
@@ -96,8 +99,17 @@ def version() -> str:
     return lib().svf_version().decode()
 
 
-def set_profiling(enabled: bool) -> None:
-    lib().svf_set_profiling(1 if enabled else 0)
+def set_profiling(mode) -> None:
+    """0/False off, 1/True phase events, 2 phase events + algorithmic work counts."""
+    lib().svf_set_profiling(int(mode))
+
+
+def simulate_work_counts():
+    """(E, U) of the last svf_simulate call made under set_profiling(2): running entries examined
+    over all head evaluations, running entries updated over all admissions."""
+    buf = (C.c_uint64 * 2)()
+    _check(lib().svf_simulate_work_counts(buf), "svf_simulate_work_counts")
+    return int(buf[0]), int(buf[1])
 
 
 def simulate_phase_ms():

@@ -20,6 +20,7 @@
 
 #include "svf_internal.cuh"
 #include "svf_state.cuh"
+#include "svf_sim_slots.cuh"
 
 namespace svf {
 
@@ -34,6 +35,7 @@ struct SimArgs {
     const uint8_t* bit;
     const uint32_t* order;           // [N] local id at (instance offset + rank)
     const uint32_t* rank;            // [N] rank of (instance offset + local id)
+    int4* req;                       // [N] (s, o, id, a) at (instance offset + rank)
     int32_t *start, *finish;
     int64_t *tel, *peak, *rounds, *decisions;
     int32_t *makespan, *status;
@@ -84,7 +86,11 @@ __global__ void __launch_bounds__(256) k_sim_rank(SimArgs g, const SortPlan* __r
         const int64_t base = __ldg(g.off + j);
         const int64_t r = p - base;
         order[p] = (uint32_t)seq;
-        if (r >= 0 && base + seq < g.N) rank[base + seq] = (uint32_t)r;
+        if (r >= 0 && base + seq < g.N) {
+            rank[base + seq] = (uint32_t)r;
+            const int64_t i = base + seq;
+            g.req[p] = make_int4(__ldg(g.s + i), __ldg(g.o + i), (int)seq, __ldg(g.a + i));
+        }
     }
 }
 
@@ -277,6 +283,8 @@ struct SimWs {
     uint64_t* words1;       // [N]
     uint32_t* order;        // [N]
     uint32_t* rank;         // [N]
+    int4* req;              // [N]
+    unsigned long long* counts;   // [2] E, U of the counting variant
     int32_t* status_tmp;    // [I] when the caller does not want status
     unsigned long long* work_ctr;
     char* gstate;
@@ -286,6 +294,9 @@ struct SimWs {
 };
 
 struct SimConfig {
+    bool slots;             // register-resident kernel (M < 2^30); else the wide sorted-array kernel
+    int ecap, qcap;         // slots kernel: ext slots per instance, bitmap capacity
+    size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
     int threads;
     bool smem;
     int cap;
@@ -295,8 +306,10 @@ struct SimConfig {
 };
 
 constexpr size_t SMEM_STATE_LIMIT = 200 * 1024;
+constexpr size_t SMEM_WARP_STATE_LIMIT = 12 * 1024;   // one-warp groups: keep >= 16 CTAs per SM
+constexpr int SLOT_K = 16;                            // register slots per thread
 
-SimConfig sim_config(const svf_trace_t* tr)
+SimConfig sim_config(const svf_trace_t* tr, int64_t M)
 {
     SimConfig c;
     const int64_t I = tr->n_instances, mx = tr->max_instance > 0 ? tr->max_instance : 1;
@@ -305,17 +318,28 @@ SimConfig sim_config(const svf_trace_t* tr)
     c.sort_lo = c.sb;
     c.sort_hi = c.sb + 32 + c.ib;
     c.cap = (int)((mx + 31) / 32 * 32);
-    const size_t sbytes = state_bytes(c.cap);
-    c.smem = sbytes <= SMEM_STATE_LIMIT;
-    c.dyn_smem = c.smem ? sbytes : 0;
+    c.slots = M < ((int64_t)1 << 30);
+    c.ecap = 0; c.qcap = c.cap;
     // group width: enough warps in flight to cover the GPU (about 16 per SM), no wider than the
     // running set can use
     const int64_t target_warps = (int64_t)sm_count() * 16;
     int64_t w = I > 0 ? target_warps / I : 1;
     int threads = 32;
-    while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
+    const int tmax = c.slots ? 256 : 1024;
+    while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
     if (threads == 64) threads = 128;
     if (threads == 512) threads = 1024;
+    if (c.slots) {
+        auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
+        if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) threads = 128;
+        c.ecap = ext_of(threads);
+        c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
+        c.smem = c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
+    } else {
+        c.state_bytes = state_bytes(c.cap);
+        c.smem = c.state_bytes <= SMEM_STATE_LIMIT;
+    }
+    c.dyn_smem = c.smem ? c.state_bytes : 0;
     c.threads = threads;
     return c;
 }
@@ -333,8 +357,38 @@ int sim_grid(const SimConfig& c, int64_t I)
     return (int)grid;
 }
 
+template <int THREADS, bool SMEM>
+int slots_grid(const SimConfig& c, int64_t I)
+{
+    int per_sm = 0;
+    if (SMEM) {
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+    }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    int64_t grid = (int64_t)per_sm * sm_count();
+    if (grid > I) grid = I;
+    if (grid < 1) grid = 1;
+    return (int)grid;
+}
+
 int sim_grid_any(const SimConfig& c, int64_t I)
 {
+    if (c.slots) {
+        if (c.smem) {
+            switch (c.threads) {
+            case 32: return slots_grid<32, true>(c, I);
+            case 128: return slots_grid<128, true>(c, I);
+            default: return slots_grid<256, true>(c, I);
+            }
+        }
+        switch (c.threads) {
+        case 32: return slots_grid<32, false>(c, I);
+        case 128: return slots_grid<128, false>(c, I);
+        default: return slots_grid<256, false>(c, I);
+        }
+    }
     if (c.smem) {
         switch (c.threads) {
         case 32: return sim_grid<32, true>(c, I);
@@ -367,9 +421,11 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
     w->words1 = (uint64_t*)(base + p); p += align_up((size_t)N * 8, 256);
     w->order = (uint32_t*)(base + p);  p += align_up((size_t)N * 4, 256);
     w->rank = (uint32_t*)(base + p);   p += align_up((size_t)N * 4, 256);
+    w->req = (int4*)(base + p);        p += align_up((size_t)N * 16, 256);
+    w->counts = (unsigned long long*)(base + p); p += 256;
     w->status_tmp = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
     w->work_ctr = (unsigned long long*)(base + p); p += 256;
-    w->slot_bytes = c.smem ? 0 : align_up(state_bytes(c.cap), 256);
+    w->slot_bytes = c.smem ? 0 : align_up(c.state_bytes, 256);
     w->grid_slots = grid_slots;
     w->gstate = base + p; p += w->slot_bytes * (size_t)grid_slots;
     w->total = p;
@@ -377,6 +433,7 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
 
 thread_local int64_t g_launches_sim = 0;
 thread_local int g_profiling = 0;
+thread_local unsigned long long* g_counts_dev = nullptr;
 thread_local bool g_events_valid = false;
 thread_local cudaEvent_t g_ev[4] = {nullptr, nullptr, nullptr, nullptr};
 
@@ -400,12 +457,16 @@ using namespace svf;
 extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr)
 {
     if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0) return 0;
-    SimConfig c = sim_config(tr);
-    SimWs w;
-    // state slots in global memory only exist for oversized instances: one CTA per SM at most
-    // 2 per SM; size for 2 x SMs (the launch never uses more)
-    sim_ws_layout(&w, nullptr, tr, c, c.smem ? 0 : 2 * sm_count());
-    return w.total + 256;
+    // M is not known here: size for the larger of the two kernels' layouts.  State slots in
+    // global memory only exist for oversized instances, at most 2 CTAs per SM.
+    size_t need = 0;
+    for (int64_t M : {(int64_t)0, (int64_t)1 << 30}) {
+        SimConfig c = sim_config(tr, M);
+        SimWs w;
+        sim_ws_layout(&w, nullptr, tr, c, c.smem ? 0 : 2 * sm_count());
+        need = w.total > need ? w.total : need;
+    }
+    return need + 256;
 }
 
 extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out,
@@ -419,7 +480,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     if (policy == SVF_SVF_1BIT && ((N > 0 && !tr->bit) || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
     if (I == 0) return SVF_OK;
     if (!tr->offsets || (N > 0 && (!tr->arrival || !tr->prompt || !tr->output))) return SVF_EINVAL;
-    SimConfig c = sim_config(tr);
+    SimConfig c = sim_config(tr, M);
     if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;          // packed sort word would not fit
     if (!ws) return SVF_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -439,7 +500,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
     g.policy = policy; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
     g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
-    g.order = w.order; g.rank = w.rank;
+    g.order = w.order; g.rank = w.rank; g.req = w.req;
     g.start = out->start; g.finish = out->finish; g.tel = out->total_latency; g.peak = out->peak_kv;
     g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
     g.status = out->status ? out->status : w.status_tmp;
@@ -462,6 +523,41 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         ++g_launches_sim;
     }
     prof_mark(1, st);
+    if (c.slots) {
+        SlotArgs q;
+        q.I = I; q.N = N; q.M = M; q.max_instance = tr->max_instance;
+        q.policy = policy; q.O0 = tr->O0; q.O1 = tr->O1;
+        q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
+        q.req = w.req; q.rank = w.rank;
+        q.start = g.start; q.finish = g.finish; q.tel = g.tel; q.peak = g.peak; q.rounds = g.rounds;
+        q.decisions = g.decisions; q.makespan = g.makespan; q.status = g.status; q.latw = g.latw;
+        q.work_ctr = w.work_ctr; q.work_counts = w.counts;
+        q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
+        const bool count = g_profiling == 2;
+        if (count) {
+            if (cudaMemsetAsync(w.counts, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
+            g_counts_dev = w.counts;
+        }
+#define SVF_SLOTS_LAUNCH(T, S)                                                            \
+        do {                                                                                  \
+            if (count) k_sim_slots<T, SLOT_K, S, true><<<grid, T, c.dyn_smem, st>>>(q);       \
+            else       k_sim_slots<T, SLOT_K, S, false><<<grid, T, c.dyn_smem, st>>>(q);      \
+        } while (0)
+        if (c.smem) {
+            switch (c.threads) {
+            case 32: SVF_SLOTS_LAUNCH(32, true); break;
+            case 128: SVF_SLOTS_LAUNCH(128, true); break;
+            default: SVF_SLOTS_LAUNCH(256, true); break;
+            }
+        } else {
+            switch (c.threads) {
+            case 32: SVF_SLOTS_LAUNCH(32, false); break;
+            case 128: SVF_SLOTS_LAUNCH(128, false); break;
+            default: SVF_SLOTS_LAUNCH(256, false); break;
+            }
+        }
+#undef SVF_SLOTS_LAUNCH
+    } else {
 #define SVF_SIM_LAUNCH(T, S) k_sim<T, S><<<grid, T, c.dyn_smem, st>>>(g)
     if (c.smem) {
         switch (c.threads) {
@@ -479,6 +575,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         }
     }
 #undef SVF_SIM_LAUNCH
+    }
     ++g_launches_sim;
     if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
     prof_mark(2, st);
@@ -498,7 +595,16 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
 }
 
-extern "C" void svf_set_profiling(int enabled) { g_profiling = enabled ? 1 : 0; }
+extern "C" void svf_set_profiling(int mode) { g_profiling = mode == 2 ? 2 : (mode ? 1 : 0); if (mode != 2) g_counts_dev = nullptr; }
+
+extern "C" int svf_simulate_work_counts(uint64_t* counts_out)
+{
+    if (!counts_out || !g_counts_dev) return SVF_EINVAL;
+    unsigned long long h[2] = {0, 0};
+    if (cudaMemcpy(h, g_counts_dev, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return SVF_ECUDA;
+    counts_out[0] = h[0]; counts_out[1] = h[1];
+    return SVF_OK;
+}
 
 extern "C" int svf_simulate_phase_ms(float* ms_out)
 {
