@@ -1,29 +1,52 @@
 // The register-resident simulator kernel (a4-a7), included by svf_simulate.cu only.
 //
 // RUNNING SET as unordered SLOTS.  Slot j of an instance holds, for one request in flight,
-//     f_j   absolute finish step (int32); the slot is DEAD (free) once f_j <= t
+//     f_j   absolute finish step (int32); the slot is DEAD (free) once f_j <= t (0 = never used)
 //     B_j   A_j + f_j  (mod 2^32), A_j = mem(f_j) of Eq. 3c for the current running set
 //     c_j   s_j - k_j  (mod 2^32)
 // The memory of a fixed set peaks at completion times only, so the set is feasible iff
 // every live A_j <= M.  Admitting h = (s_h, o_h) at time t, f_h = t + o_h:
-//     (1)  A_h = s_h + o_h + sum_{f_i >= f_h} (c_i + t) + #{f_i >= f_h} o_h        <= M
+//     (1)  A_h = s_h + o_h + sum_{f_i >= f_h} (c_i + f_h)                            <= M
 //     (2)  for every live j with f_j <= f_h:   A_j + s_h + (f_j - t)                <= M
 // and on admission every such j gets A_j += s_h + f_j - t.  Nothing depends on the ORDER of
-// the slots: no sorted array, no shifting; a pass is a flat loop over slots, the first
-// THREADS*K of which live in REGISTERS (slot k*THREADS + tid is register k of thread tid); the
-// rest (only when more than THREADS*K requests run at once) sit in an `ext` array that is
-// only ever touched by the owning thread.  One reduction (and, for a multi-warp group, one
-// barrier) per evaluation.
+// the slots: no sorted array, no shifting; a pass is straight-line code over the slots, the
+// first THREADS*K of which live in REGISTERS (slot k*THREADS + tid is register k of thread
+// tid); the rest (only when more than THREADS*K requests run at once) sit in an `ext` array
+// that is only ever touched by the owning thread.
+//
+// Per slot the EVALUATION pass costs six integer instructions:
+//     x = f - (t+1)            as unsigned: x < 2^31 iff the slot is live (f > t)
+//     in = x <u o_h            live and f <= f_h            (condition (2) applies)
+//     ge = f >= f_h            (a dead slot has f <= t < f_h)
+//     if (ge) acc += c + f_h   one IADD3                    (condition (1))
+//     if (in) viol = max(viol, B + (s_h - t - M))           one VIADDMNMX
+//     dead-bit of x shifted into a mask                     (free-slot search, one SHF)
+// the UPDATE pass three (x, in, B += s_h - t + f), and a BLOCKED head costs one more pass that
+// finds how long it must stay blocked (below).  One reduction round per pass.
 //
 // Arithmetic is 32 bit, wrapping: every TRUE value that is compared lies in [-M, 2M] and the
 // host takes this kernel only when M < 2^30, so the wrapped result read as int32 is exact.
 // peak_kv = max over all A values ever produced (each entry's final A_j is mem(f_j)).
 //
-// WAITING QUEUE: two-level bitmap over ranks (keys are time-invariant, so the presort fixes
-// the order); the two lowest waiting ranks with their (s, o, id, a) are cached in registers:
-// `head` and `second` (second's record is fetched one admission ahead, hiding the L2 latency).
-// ARRIVALS come from a 32-wide register window over (a, s, o, rank), refilled once per 32
-// arrivals; an arrival that becomes head/second takes its record from the window.
+// TIME ADVANCE (exact, R1/R16).  Completions are implicit.  With an empty queue nothing can
+// happen before the next arrival.  A BLOCKED head h stays blocked while the running set only
+// shrinks (nobody may bypass it), and each obstacle has a closed-form end:
+//   * a violated (2) at slot j clears at min(f_j, t + v_j), v_j = A_j + s_h + f_j - t - M (it
+//     relaxes by one token per step; A_j is fixed while nothing is admitted);
+//   * a violated (1) holds at least until the first of the summed slots drops out of the sum:
+//     t' + o_h > min{f_i : f_i >= f_h}.
+// The head is re-evaluated at t_lb = the latest of these ends, or earlier if an arrival takes
+// its place at the head of the queue; the steps in between are counted into rounds/decisions
+// exactly as the step-by-step definition counts them (one blocked-head evaluation each).
+//
+// WAITING QUEUE: bitmap over ranks (keys are time-invariant, so the presort fixes the order):
+// one 32-bit word per lane in a register when the instance has at most 1024 requests (QREG),
+// else the two-level shared-memory bitmap of svf_state.cuh.  The two lowest waiting ranks with
+// their (s, o, id, a) are cached in registers: `head` and `second` (second's record is fetched
+// one admission ahead, hiding the L2 latency).  ARRIVALS come from a 32-wide register window
+// over (a, s, o, rank), refilled once per 32 arrivals; an arrival that becomes head/second
+// takes its record from the window.  OUTPUTS (start, finish, latency word) are buffered one
+// admission per lane and written 32 at a time.
 #pragma once
 
 #include <limits.h>
@@ -71,6 +94,20 @@ __device__ __forceinline__ int queue_first_ge(const uint32_t* L0, const uint32_t
     }
 }
 
+// the register bitmap (QREG): lane l holds ranks [32 l, 32 l + 32).  Smallest set bit >= q.
+__device__ __forceinline__ int qreg_first_ge(uint32_t word, int q)
+{
+    const int lane = threadIdx.x & 31;
+    const int w0 = q >> 5;
+    if (lane == w0) word &= ~0u << (q & 31);
+    if (lane < w0) word = 0u;
+    const uint32_t b = __ballot_sync(FULL, word != 0u);
+    if (!b) return INT_MAX;
+    const int l = __ffs(b) - 1;
+    const uint32_t wv = __shfl_sync(FULL, word, l);
+    return l * 32 + (__ffs(wv) - 1);
+}
+
 struct SlotArgs {
     int64_t I, N, M, max_instance;
     int policy; int32_t O0, O1;
@@ -96,68 +133,57 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
     return align_up((size_t)nL0 * 4, 16) + align_up((size_t)nL1 * 4, 16) + 3 * align_up((size_t)ecap * 4, 16);
 }
 
-
-// the five results of one evaluation pass, reduced over the group (uniform afterwards)
-struct EvalRed { int cnt; uint32_t csum; int viol; int minf; int fidx; };
-
+// one reduction round over the group: a summed (mod 2^32), b maxed, c minned; uniform afterwards
 template <int THREADS>
-__device__ __forceinline__ void reduce_eval(EvalRed& r, int (*red)[THREADS / 32][5], int& parity)
+__device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, int (*red)[THREADS / 32][3], int& parity)
 {
-    r.cnt = __reduce_add_sync(FULL, r.cnt);
-    r.csum = __reduce_add_sync(FULL, r.csum);
-    r.viol = __reduce_max_sync(FULL, r.viol);
-    r.minf = __reduce_min_sync(FULL, r.minf);
-    r.fidx = __reduce_min_sync(FULL, r.fidx);
+    a = __reduce_add_sync(FULL, a);
+    b = __reduce_max_sync(FULL, b);
+    c = __reduce_min_sync(FULL, c);
     if (THREADS > 32) {
         constexpr int WARPS = THREADS / 32;
         const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-        int (*sc)[5] = red[parity];
+        int (*sc)[3] = red[parity];
         parity ^= 1;
-        if (lane == 0) { sc[wrp][0] = r.cnt; sc[wrp][1] = (int)r.csum; sc[wrp][2] = r.viol; sc[wrp][3] = r.minf; sc[wrp][4] = r.fidx; }
+        if (lane == 0) { sc[wrp][0] = (int)a; sc[wrp][1] = b; sc[wrp][2] = c; }
         __syncthreads();
         const bool in = lane < WARPS;
         const int l = in ? lane : 0;
-        r.cnt = __reduce_add_sync(FULL, in ? sc[l][0] : 0);
-        r.csum = __reduce_add_sync(FULL, in ? (uint32_t)sc[l][1] : 0u);
-        r.viol = __reduce_max_sync(FULL, in ? sc[l][2] : INT_MIN);
-        r.minf = __reduce_min_sync(FULL, in ? sc[l][3] : INT_MAX);
-        r.fidx = __reduce_min_sync(FULL, in ? sc[l][4] : INT_MAX);
+        a = __reduce_add_sync(FULL, in ? (uint32_t)sc[l][0] : 0u);
+        b = __reduce_max_sync(FULL, in ? sc[l][1] : INT_MIN);
+        c = __reduce_min_sync(FULL, in ? sc[l][2] : INT_MAX);
     }
 }
 
-// min over the group of one value (the next completion time when no evaluation ran this step)
-template <int THREADS>
-__device__ __forceinline__ int reduce_min1(int v, int (*red)[THREADS / 32][5], int& parity)
-{
-    v = __reduce_min_sync(FULL, v);
-    if (THREADS > 32) {
-        constexpr int WARPS = THREADS / 32;
-        const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-        int (*sc)[5] = red[parity];
-        parity ^= 1;
-        if (lane == 0) sc[wrp][0] = v;
-        __syncthreads();
-        v = __reduce_min_sync(FULL, lane < WARPS ? sc[lane][0] : INT_MAX);
+// straight-line code over register slots kmax-1 .. 0 (one indexed branch, no loop overhead)
+#define SVF_SLOT_SWITCH(kmax, OP)                                                             \
+    switch (kmax) {                                                                           \
+    default:                                                                                  \
+    case 16: OP(15) case 15: OP(14) case 14: OP(13) case 13: OP(12)                           \
+    case 12: OP(11) case 11: OP(10) case 10: OP(9)  case 9:  OP(8)                            \
+    case 8:  OP(7)  case 7:  OP(6)  case 6:  OP(5)  case 5:  OP(4)                            \
+    case 4:  OP(3)  case 3:  OP(2)  case 2:  OP(1)  case 1:  OP(0)                            \
+    case 0: break;                                                                            \
     }
-    return v;
-}
 
-
-template <int THREADS, int K, bool SMEM, bool COUNT>
+template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
 __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
 {
+    static_assert(K == 16, "SVF_SLOT_SWITCH is written out for 16 register slots per thread");
     using G = Group<THREADS>;
     constexpr int WARPS = THREADS / 32;
     constexpr int REGCAP = THREADS * K;
+    constexpr int TSHIFT = THREADS == 32 ? 5 : (THREADS == 128 ? 7 : 8);
+    static_assert((1 << TSHIFT) == THREADS, "THREADS must be 32, 128 or 256");
     extern __shared__ __align__(16) char dyn_smem[];
     __shared__ int scratch[2][64];
-    __shared__ int red[2][WARPS][5];
+    __shared__ int red[2][WARPS][3];
     __shared__ long long inst_s;
     int parity = 0, rparity = 0;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
 
     char* sbase = SMEM ? dyn_smem : g.gstate + (size_t)blockIdx.x * g.slot_bytes;
-    const int capL0 = (g.qcap + 31) / 32, capL1 = (capL0 + 31) / 32;
+    const int capL0 = QREG ? 0 : (g.qcap + 31) / 32, capL1 = (capL0 + 31) / 32;
     uint32_t* L0 = reinterpret_cast<uint32_t*>(sbase);
     uint32_t* L1 = reinterpret_cast<uint32_t*>(sbase + align_up((size_t)capL0 * 4, 16));
     char* ebase = reinterpret_cast<char*>(L1) + align_up((size_t)capL1 * 4, 16);
@@ -165,7 +191,8 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     int32_t* ef = reinterpret_cast<int32_t*>(ebase);
     uint32_t* eB = reinterpret_cast<uint32_t*>(ebase + estride);
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
-    const uint32_t Mu = (uint32_t)g.M;
+    const int Mi = (int)g.M;
+    const bool want_start = g.start != nullptr, want_finish = g.finish != nullptr, want_latw = g.latw != nullptr;
 
     while (true) {
         if (tid == 0) inst_s = (long long)atomicAdd(g.work_ctr, 1ull);
@@ -204,26 +231,34 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         if ((int64_t)max_a + sum_o >= ((int64_t)1 << 31)) flags |= F_OVERFLOW;   // horizon
         const int32_t status = status_from_flags(flags);
 
-        int64_t tel = 0, peak = 0, rounds = 0, decisions = 0;
-        int32_t mk = 0;
+        int64_t tel = 0;                 // per-lane partial sums (warp 0), reduced at the end
+        int mk = 0, peak = 0;
+        uint32_t rounds = 0, decisions = 0;
         long long cntE = 0, cntU = 0;
 
         if (status != SVF_OK || n == 0) {
             for (int i = tid; i < n; i += THREADS) {
-                if (g.start) g.start[base + i] = -1;
-                if (g.finish) g.finish[base + i] = -1;
-                if (g.latw) g.latw[base + i] = (uint64_t)j << 32;
+                if (want_start) g.start[base + i] = -1;
+                if (want_finish) g.finish[base + i] = -1;
+                if (want_latw) g.latw[base + i] = (uint64_t)j << 32;
             }
         } else {
             const uint32_t* __restrict__ rnk = g.rank + base;
             const int4* __restrict__ req = g.req + base;
+            int32_t* __restrict__ out_start = g.start + base;
+            int32_t* __restrict__ out_finish = g.finish + base;
+            uint64_t* __restrict__ out_latw = g.latw + base;
+            const uint64_t jhi = (uint64_t)j << 32;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
-            for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
-            for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
+            uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32)
+            if (!QREG) {
+                for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
+                for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
+            }
 
             int f[K]; uint32_t B[K], c[K];
 #pragma unroll
-            for (int k = 0; k < K; ++k) { f[k] = INT_MIN; B[k] = 0; c[k] = 0; }
+            for (int k = 0; k < K; ++k) { f[k] = 0; B[k] = 0; c[k] = 0; }
 
             // arrival window: lane l holds request wb + l
             int wb = 0, aw, sw, ow, rw;
@@ -238,13 +273,25 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 Rec x; x.r = r; x.s = __shfl_sync(FULL, sw, l); x.o = __shfl_sync(FULL, ow, l);
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
             };
-            G::sync();
+            // output buffer: admission number m sits in lane m % 32 of warp 0 until 32 are there
+            int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
+            auto flush = [&](int count) {
+                if (wrp == 0 && lane < count) {
+                    if (want_start) out_start[b_id] = b_t;
+                    if (want_finish) out_finish[b_id] = b_f;
+                    if (want_latw) out_latw[b_id] = jhi | (uint32_t)b_lat;
+                    tel += b_lat;
+                    mk = b_f > mk ? b_f : mk;
+                }
+            };
+            if (!QREG) G::sync();
 
             Rec head, second;
             head.r = INT_MAX; head.s = head.o = head.id = head.a = 0;
             second = head;
-            int next = 0, started = 0, hw = 0, minf = INT_MAX;
+            int next = 0, started = 0, hw = 0;
             int32_t t = a[0];
+            int32_t t_lb = t;                     // first step at which the head must be (re)evaluated
 
             while (started < n) {
                 // 2. ARRIVE (1. COMPLETE is implicit: a slot is dead once f <= t)
@@ -255,140 +302,171 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                     const bool v = idx >= next && aw <= t;
                     const uint32_t m = __ballot_sync(FULL, v);
                     if (!m) break;
-                    // nobody may still be reading the bitmap for the previous step
-                    if (!arrived) G::sync();
+                    if (QREG) {
+                        for (uint32_t mm = m; mm; mm &= mm - 1u) {
+                            const int r = __shfl_sync(FULL, rw, __ffs(mm) - 1);
+                            if (lane == (r >> 5)) qword |= 1u << (r & 31);
+                        }
+                    } else {
+                        // nobody may still be reading the bitmap for the previous step
+                        if (!arrived) G::sync();
+                        if (wrp == 0 && v) queue_set(L0, L1, rw);
+                    }
                     arrived = true;
-                    if (wrp == 0 && v) queue_set(L0, L1, rw);
                     const int r1 = __reduce_min_sync(FULL, v ? rw : INT_MAX);
-                    const int l1 = __ffs(__ballot_sync(FULL, v && rw == r1)) - 1;
-                    const int r2 = __reduce_min_sync(FULL, (v && lane != l1) ? rw : INT_MAX);
-                    const uint32_t b2 = __ballot_sync(FULL, v && lane != l1 && rw == r2);
-                    const int l2 = b2 ? __ffs(b2) - 1 : 0;
-                    if (r1 < head.r) {
-                        const Rec n1 = win_rec(l1, r1);
-                        if (r2 < head.r) second = win_rec(l2, r2); else second = head;
-                        head = n1;
-                    } else if (r1 < second.r) {
-                        second = win_rec(l1, r1);
+                    if (r1 < second.r) {
+                        const int l1 = __ffs(__ballot_sync(FULL, v && rw == r1)) - 1;
+                        if (r1 < head.r) {
+                            const int r2 = __reduce_min_sync(FULL, (v && lane != l1) ? rw : INT_MAX);
+                            const Rec n1 = win_rec(l1, r1);
+                            if (r2 < head.r) {
+                                const int l2 = __ffs(__ballot_sync(FULL, v && lane != l1 && rw == r2)) - 1;
+                                second = win_rec(l2, r2);
+                            } else {
+                                second = head;
+                            }
+                            head = n1;
+                            t_lb = t;                 // a new head: evaluate it now
+                        } else {
+                            second = win_rec(l1, r1);
+                        }
                     }
                     next += __popc(m);
                     if (next < wb + 32) break;
                 }
-                if (arrived && THREADS == 32) __syncwarp();
+                if (!QREG && arrived && THREADS == 32) __syncwarp();
 
                 // 3. ADMIT
-                int64_t wait = 1;
                 if (head.r != INT_MAX) {
                     rounds += 1;
-                    while (head.r != INT_MAX) {
+                    while (t >= t_lb) {
+                        // ---- evaluation pass -----------------------------------------------------
                         const int fh = t + head.o;
-                        const uint32_t Kc = (uint32_t)head.s - (uint32_t)t - Mu;
-                        EvalRed e; e.cnt = 0; e.csum = 0; e.viol = INT_MIN; e.minf = INT_MAX; e.fidx = INT_MAX;
-                        int kmax = (hw + THREADS - 1) / THREADS; kmax = kmax < K ? kmax : K;
-                        int fr = INT_MAX;
-#pragma unroll
-                        for (int k = 0; k < K; ++k) {
-                            if (k >= kmax) break;
-                            const int fk = f[k];
-                            const bool live = fk > t, ge = fk >= fh;
-                            if (ge) { e.cnt += 1; e.csum += c[k]; }
-                            const int v = (int)(B[k] + Kc);
-                            if (live && fk <= fh) e.viol = v > e.viol ? v : e.viol;
-                            if (live) e.minf = fk < e.minf ? fk : e.minf;
-                            else fr = fr < k ? fr : k;
-                            if (COUNT) cntE += live;
+                        const uint32_t t1 = (uint32_t)t + 1u, oh = (uint32_t)head.o, fhu = (uint32_t)fh;
+                        const uint32_t Kc = (uint32_t)head.s - (uint32_t)t - (uint32_t)Mi;   // s_h - t - M (mod 2^32)
+                        uint32_t acc = 0, dm = 0;
+                        int viol = INT_MIN;
+                        int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;
+#define SVF_EVAL(k) {                                                                          \
+                            const uint32_t x = (uint32_t)f[k] - t1;                            \
+                            if (f[k] >= fh) acc += c[k] + fhu;                                 \
+                            if (x < oh) viol = __viaddmax_s32((int)B[k], (int)Kc, viol);            \
+                            dm = __funnelshift_l(x, dm, 1);                                    \
+                            if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
                         }
-                        if (fr != INT_MAX) e.fidx = fr * THREADS + tid;
+                        SVF_SLOT_SWITCH(kmax, SVF_EVAL)
+#undef SVF_EVAL
+                        // lowest free register slot of this thread: bit k of dm = slot k is dead
+                        const int kfree = dm ? __ffs(dm) - 1 : kmax;
+                        int fidx = kfree < K ? (kfree << TSHIFT) + tid : INT_MAX;
                         for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                            const int x = q - REGCAP;
-                            const int fk = ef[x];
-                            const bool live = fk > t, ge = fk >= fh;
-                            if (ge) { e.cnt += 1; e.csum += ec[x]; }
-                            const int v = (int)(eB[x] + Kc);
-                            if (live && fk <= fh) e.viol = v > e.viol ? v : e.viol;
-                            if (live) e.minf = fk < e.minf ? fk : e.minf;
-                            else e.fidx = e.fidx < q ? e.fidx : q;
-                            if (COUNT) cntE += live;
+                            const int e = q - REGCAP;
+                            const int fk = ef[e];
+                            const uint32_t x = (uint32_t)fk - t1;
+                            if (fk >= fh) acc += ec[e] + fhu;
+                            if (x < oh) viol = __viaddmax_s32((int)eB[e], (int)Kc, viol);
+                            if (x >> 31) fidx = fidx < q ? fidx : q;
+                            if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
                         }
-                        reduce_eval<THREADS>(e, red, rparity);
-                        minf = e.minf;
-                        const int S = (int)(e.csum + (uint32_t)e.cnt * (uint32_t)t);
-                        const int64_t Ah = (int64_t)head.s + head.o + S + (int64_t)e.cnt * head.o;
-                        const bool ok2 = e.viol <= 0;
-                        if (!(ok2 && Ah <= g.M)) { wait = ok2 ? 1 : e.viol; break; }   // blocked: no bypass
+                        reduce_add_max_min<THREADS>(acc, viol, fidx, red, rparity);
+                        const int Ah = head.s + head.o + (int)acc;        // exact: 0 <= A_h <= 2M < 2^31
+                        if (viol > 0 || Ah > Mi) {
+                            // ---- blocked (no bypass): how long at least? ------------------
+                            int wmax = 0, minge = INT_MAX;
+#define SVF_BLOCK(k) {                                                                         \
+                                const uint32_t x = (uint32_t)f[k] - t1;                        \
+                                const int v = (int)(B[k] + Kc), d = (int)x + 1;                  \
+                                const int w = v < d ? v : d;                                   \
+                                if (x < oh) wmax = w > wmax ? w : wmax;                        \
+                                if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
+                            }
+                            SVF_SLOT_SWITCH(kmax, SVF_BLOCK)
+#undef SVF_BLOCK
+                            for (int q = REGCAP + tid; q < hw; q += THREADS) {
+                                const int e = q - REGCAP;
+                                const int fk = ef[e];
+                                const uint32_t x = (uint32_t)fk - t1;
+                                const int v = (int)(eB[e] + Kc), d = (int)x + 1;
+                                const int w = v < d ? v : d;
+                                if (x < oh) wmax = w > wmax ? w : wmax;
+                                if (fk >= fh) minge = fk < minge ? fk : minge;
+                            }
+                            uint32_t z = 0;
+                            reduce_add_max_min<THREADS>(z, wmax, minge, red, rparity);
+                            int lb = t + (wmax > 1 ? wmax : 1);
+                            if (Ah > Mi) { const int l1 = minge - head.o + 1; lb = l1 > lb ? l1 : lb; }
+                            t_lb = lb;
+                            break;
+                        }
 
-                        // admit the head into slot idx
-                        const int idx = e.fidx == INT_MAX ? hw : e.fidx;
-                        hw = idx + 1 > hw ? idx + 1 : hw;
+                        // ---- admit the head: update pass, then write it into slot idx ------------
+                        const int idx = fidx == INT_MAX ? hw : fidx;
                         const uint32_t add = (uint32_t)head.s - (uint32_t)t;
-                        const uint32_t Bh = (uint32_t)Ah + (uint32_t)fh;
-                        kmax = (hw + THREADS - 1) / THREADS; kmax = kmax < K ? kmax : K;
-                        const int myk = (idx < REGCAP && (idx % THREADS) == tid) ? idx / THREADS : -1;
-#pragma unroll
-                        for (int k = 0; k < K; ++k) {
-                            if (k >= kmax) break;
-                            const int fk = f[k];
-                            if (fk > t && fk <= fh) { B[k] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
-                            if (k == myk) { f[k] = fh; B[k] = Bh; c[k] = add; }
+                        const uint32_t Bh = (uint32_t)Ah + fhu;
+#define SVF_UPDATE(k) {                                                                        \
+                            const uint32_t x = (uint32_t)f[k] - t1;                            \
+                            if (x < oh) { B[k] += add + (uint32_t)f[k]; if (COUNT) cntU += 1; } \
                         }
+                        SVF_SLOT_SWITCH(kmax, SVF_UPDATE)
+#undef SVF_UPDATE
                         for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                            const int x = q - REGCAP;
-                            const int fk = ef[x];
-                            if (fk > t && fk <= fh) { eB[x] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
-                            if (q == idx) { ef[x] = fh; eB[x] = Bh; ec[x] = add; }
+                            const int e = q - REGCAP;
+                            const int fk = ef[e];
+                            if ((uint32_t)fk - t1 < oh) { eB[e] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
                         }
-                        minf = fh < minf ? fh : minf;
-                        peak = Ah > peak ? Ah : peak;
-                        if (e.viol != INT_MIN) { const int64_t pj = g.M + e.viol; peak = pj > peak ? pj : peak; }
-                        if (tid == 0) {
-                            queue_clear(L0, L1, head.r);
-                            if (g.start) g.start[base + head.id] = t;
-                            if (g.finish) g.finish[base + head.id] = fh;
-                            if (g.latw) g.latw[base + head.id] = ((uint64_t)j << 32) | (uint32_t)(fh - head.a);
+                        if (idx < REGCAP) {
+                            const bool mine = (idx & (THREADS - 1)) == tid;
+#define SVF_PUT(k) { if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; } break; }
+                            switch (idx >> TSHIFT) {
+                            case 0: SVF_PUT(0) case 1: SVF_PUT(1) case 2: SVF_PUT(2) case 3: SVF_PUT(3)
+                            case 4: SVF_PUT(4) case 5: SVF_PUT(5) case 6: SVF_PUT(6) case 7: SVF_PUT(7)
+                            case 8: SVF_PUT(8) case 9: SVF_PUT(9) case 10: SVF_PUT(10) case 11: SVF_PUT(11)
+                            case 12: SVF_PUT(12) case 13: SVF_PUT(13) case 14: SVF_PUT(14) default: SVF_PUT(15)
+                            }
+#undef SVF_PUT
+                        } else if (((idx - REGCAP) & (THREADS - 1)) == tid) {
+                            const int e = idx - REGCAP;
+                            ef[e] = fh; eB[e] = Bh; ec[e] = add;
                         }
-                        tel += fh - head.a;
-                        mk = fh > mk ? fh : mk;
+                        hw = idx + 1 > hw ? idx + 1 : hw;
+                        {   // every final A_j is a mem(f_j): the new A_h and the raised in-range A_j
+                            const int pj = Mi + viol;                  // INT_MIN + M: no in-range slot
+                            const int p2 = Ah > pj ? Ah : pj;
+                            peak = p2 > peak ? p2 : peak;
+                        }
+                        if (QREG) { if (lane == (head.r >> 5)) qword &= ~(1u << (head.r & 31)); }
+                        else if (tid == 0) queue_clear(L0, L1, head.r);
+                        if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
                         ++started; ++decisions;
+                        if ((started & 31) == 0) flush(32);
                         // promote the second; fetch the record behind it one admission ahead
                         head = second;
                         second.r = INT_MAX;
-                        if (head.r != INT_MAX) {
-                            const int r = queue_first_ge(L0, L1, n, nL1, head.r + 1);
-                            if (r != INT_MAX) {
-                                const int4 qv = req[r];
-                                second.r = r; second.s = qv.x; second.o = qv.y; second.id = qv.z; second.a = qv.w;
-                            }
+                        if (head.r == INT_MAX) break;
+                        const int r = QREG ? qreg_first_ge(qword, head.r + 1)
+                                           : queue_first_ge(L0, L1, n, nL1, head.r + 1);
+                        if (r != INT_MAX) {
+                            const int4 qv = req[r];
+                            second.r = r; second.s = qv.x; second.o = qv.y; second.id = qv.z; second.a = qv.w;
                         }
                     }
-                    if (head.r != INT_MAX) ++decisions;          // one blocked-head evaluation
+                    if (head.r != INT_MAX) ++decisions;          // one blocked-head evaluation (R16)
                 }
                 if (started == n) break;
                 // 4. ADVANCE to the next step at which anything can change (exact, R16)
-                int64_t t_arr = INT_MAX;
+                int tn = INT_MAX;
                 if (next < n) {
                     if (next >= wb + 32) { wb = next; load_window(); }
-                    t_arr = __shfl_sync(FULL, aw, next - wb);
+                    tn = __shfl_sync(FULL, aw, next - wb);
                 }
-                if (minf <= t) {          // the earliest finisher completed and nothing was evaluated since
-                    int kmax = (hw + THREADS - 1) / THREADS; kmax = kmax < K ? kmax : K;
-                    int mf = INT_MAX;
-#pragma unroll
-                    for (int k = 0; k < K; ++k) {
-                        if (k >= kmax) break;
-                        if (f[k] > t) mf = f[k] < mf ? f[k] : mf;
-                    }
-                    for (int q = REGCAP + tid; q < hw; q += THREADS) { const int fk = ef[q - REGCAP]; if (fk > t) mf = fk < mf ? fk : mf; }
-                    minf = reduce_min1<THREADS>(mf, red, rparity);
-                }
-                int64_t tn = t_arr < (int64_t)minf ? t_arr : (int64_t)minf;
                 if (head.r != INT_MAX) {                      // blocked head waits
-                    const int64_t t_lb = (int64_t)t + wait;
                     tn = t_lb < tn ? t_lb : tn;
-                    rounds += tn - t - 1;
-                    decisions += tn - t - 1;
+                    rounds += (uint32_t)(tn - t - 1);
+                    decisions += (uint32_t)(tn - t - 1);
                 }
-                t = (int32_t)tn;
+                t = tn;
             }
+            flush(started & 31);
         }
         if (COUNT) {
 #pragma unroll
@@ -398,11 +476,16 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 atomicAdd(&g.work_counts[1], (unsigned long long)cntU);
             }
         }
+        if (wrp == 0) {
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) tel += __shfl_xor_sync(FULL, tel, d);
+            mk = __reduce_max_sync(FULL, mk);
+        }
         if (tid == 0) {
             if (g.tel) g.tel[j] = tel;
-            if (g.peak) g.peak[j] = peak;
-            if (g.rounds) g.rounds[j] = rounds;
-            if (g.decisions) g.decisions[j] = decisions;
+            if (g.peak) g.peak[j] = (int64_t)peak;
+            if (g.rounds) g.rounds[j] = (int64_t)rounds;
+            if (g.decisions) g.decisions[j] = (int64_t)decisions;
             if (g.makespan) g.makespan[j] = mk;
             if (g.status) g.status[j] = status;
         }

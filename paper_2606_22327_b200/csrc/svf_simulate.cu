@@ -296,6 +296,7 @@ struct SimWs {
 struct SimConfig {
     bool slots;             // register-resident kernel (M < 2^30); else the wide sorted-array kernel
     int ecap, qcap;         // slots kernel: ext slots per instance, bitmap capacity
+    bool qreg;              // slots kernel: waiting bitmap in one register per lane (<= 1024 ranks)
     size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
     int threads;
     bool smem;
@@ -319,7 +320,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M)
     c.sort_hi = c.sb + 32 + c.ib;
     c.cap = (int)((mx + 31) / 32 * 32);
     c.slots = M < ((int64_t)1 << 30);
-    c.ecap = 0; c.qcap = c.cap;
+    c.ecap = 0; c.qcap = c.cap; c.qreg = false;
     // group width: enough warps in flight to cover the GPU (about 16 per SM), no wider than the
     // running set can use
     const int64_t target_warps = (int64_t)sm_count() * 16;
@@ -331,10 +332,12 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M)
     if (threads == 512) threads = 1024;
     if (c.slots) {
         auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
+        c.qreg = mx <= 1024;
+        if (c.qreg) c.qcap = 0;
         if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) threads = 128;
         c.ecap = ext_of(threads);
         c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
-        c.smem = c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
+        c.smem = c.qreg || c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
     } else {
         c.state_bytes = state_bytes(c.cap);
         c.smem = c.state_bytes <= SMEM_STATE_LIMIT;
@@ -357,15 +360,15 @@ int sim_grid(const SimConfig& c, int64_t I)
     return (int)grid;
 }
 
-template <int THREADS, bool SMEM>
+template <int THREADS, bool SMEM, bool QREG>
 int slots_grid(const SimConfig& c, int64_t I)
 {
     int per_sm = 0;
     if (SMEM) {
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true, QREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
     }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
     int64_t grid = (int64_t)per_sm * sm_count();
     if (grid > I) grid = I;
@@ -376,17 +379,24 @@ int slots_grid(const SimConfig& c, int64_t I)
 int sim_grid_any(const SimConfig& c, int64_t I)
 {
     if (c.slots) {
+        if (c.qreg) {
+            switch (c.threads) {
+            case 32: return slots_grid<32, true, true>(c, I);
+            case 128: return slots_grid<128, true, true>(c, I);
+            default: return slots_grid<256, true, true>(c, I);
+            }
+        }
         if (c.smem) {
             switch (c.threads) {
-            case 32: return slots_grid<32, true>(c, I);
-            case 128: return slots_grid<128, true>(c, I);
-            default: return slots_grid<256, true>(c, I);
+            case 32: return slots_grid<32, true, false>(c, I);
+            case 128: return slots_grid<128, true, false>(c, I);
+            default: return slots_grid<256, true, false>(c, I);
             }
         }
         switch (c.threads) {
-        case 32: return slots_grid<32, false>(c, I);
-        case 128: return slots_grid<128, false>(c, I);
-        default: return slots_grid<256, false>(c, I);
+        case 32: return slots_grid<32, false, false>(c, I);
+        case 128: return slots_grid<128, false, false>(c, I);
+        default: return slots_grid<256, false, false>(c, I);
         }
     }
     if (c.smem) {
@@ -538,22 +548,28 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
             if (cudaMemsetAsync(w.counts, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
             g_counts_dev = w.counts;
         }
-#define SVF_SLOTS_LAUNCH(T, S)                                                            \
+#define SVF_SLOTS_LAUNCH(T, S, Q)                                                         \
         do {                                                                                  \
-            if (count) k_sim_slots<T, SLOT_K, S, true><<<grid, T, c.dyn_smem, st>>>(q);       \
-            else       k_sim_slots<T, SLOT_K, S, false><<<grid, T, c.dyn_smem, st>>>(q);      \
+            if (count) k_sim_slots<T, SLOT_K, S, true, Q><<<grid, T, c.dyn_smem, st>>>(q);    \
+            else       k_sim_slots<T, SLOT_K, S, false, Q><<<grid, T, c.dyn_smem, st>>>(q);   \
         } while (0)
-        if (c.smem) {
+        if (c.qreg) {
             switch (c.threads) {
-            case 32: SVF_SLOTS_LAUNCH(32, true); break;
-            case 128: SVF_SLOTS_LAUNCH(128, true); break;
-            default: SVF_SLOTS_LAUNCH(256, true); break;
+            case 32: SVF_SLOTS_LAUNCH(32, true, true); break;
+            case 128: SVF_SLOTS_LAUNCH(128, true, true); break;
+            default: SVF_SLOTS_LAUNCH(256, true, true); break;
+            }
+        } else if (c.smem) {
+            switch (c.threads) {
+            case 32: SVF_SLOTS_LAUNCH(32, true, false); break;
+            case 128: SVF_SLOTS_LAUNCH(128, true, false); break;
+            default: SVF_SLOTS_LAUNCH(256, true, false); break;
             }
         } else {
             switch (c.threads) {
-            case 32: SVF_SLOTS_LAUNCH(32, false); break;
-            case 128: SVF_SLOTS_LAUNCH(128, false); break;
-            default: SVF_SLOTS_LAUNCH(256, false); break;
+            case 32: SVF_SLOTS_LAUNCH(32, false, false); break;
+            case 128: SVF_SLOTS_LAUNCH(128, false, false); break;
+            default: SVF_SLOTS_LAUNCH(256, false, false); break;
             }
         }
 #undef SVF_SLOTS_LAUNCH
