@@ -155,14 +155,17 @@ __device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, 
     }
 }
 
-// straight-line code over register slots kmax-1 .. 0 (one indexed branch, no loop overhead)
-#define SVF_SLOT_SWITCH(kmax, OP)                                                             \
-    switch (kmax) {                                                                           \
+// straight-line code over register slots 4*g4-1 .. 0 (g4 = groups of four slots in use): one
+// indexed branch, no loop overhead; four slots per basic block so that the compiler can
+// interleave their dependent chains (x -> compare -> predicated op).  A slot past the high-water
+// mark is dead (f = 0) and costs its instructions only.
+#define SVF_SLOT_SWITCH(g4, OP)                                                               \
+    switch (g4) {                                                                             \
     default:                                                                                  \
-    case 16: OP(15) case 15: OP(14) case 14: OP(13) case 13: OP(12)                           \
-    case 12: OP(11) case 11: OP(10) case 10: OP(9)  case 9:  OP(8)                            \
-    case 8:  OP(7)  case 7:  OP(6)  case 6:  OP(5)  case 5:  OP(4)                            \
-    case 4:  OP(3)  case 3:  OP(2)  case 2:  OP(1)  case 1:  OP(0)                            \
+    case 4: OP(15) OP(14) OP(13) OP(12)                                                       \
+    case 3: OP(11) OP(10) OP(9)  OP(8)                                                        \
+    case 2: OP(7)  OP(6)  OP(5)  OP(4)                                                        \
+    case 1: OP(3)  OP(2)  OP(1)  OP(0)                                                        \
     case 0: break;                                                                            \
     }
 
@@ -346,7 +349,8 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                         const uint32_t Kc = (uint32_t)head.s - (uint32_t)t - (uint32_t)Mi;   // s_h - t - M (mod 2^32)
                         uint32_t acc = 0, dm = 0;
                         int viol = INT_MIN;
-                        int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;
+                        int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
+                        const int g4 = (kmax + 3) >> 2;
 #define SVF_EVAL(k) {                                                                          \
                             const uint32_t x = (uint32_t)f[k] - t1;                            \
                             if (f[k] >= fh) acc += c[k] + fhu;                                 \
@@ -354,10 +358,10 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             dm = __funnelshift_l(x, dm, 1);                                    \
                             if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
                         }
-                        SVF_SLOT_SWITCH(kmax, SVF_EVAL)
+                        SVF_SLOT_SWITCH(g4, SVF_EVAL)
 #undef SVF_EVAL
                         // lowest free register slot of this thread: bit k of dm = slot k is dead
-                        const int kfree = dm ? __ffs(dm) - 1 : kmax;
+                        const int kfree = dm ? __ffs(dm) - 1 : 4 * g4;
                         int fidx = kfree < K ? (kfree << TSHIFT) + tid : INT_MAX;
                         for (int q = REGCAP + tid; q < hw; q += THREADS) {
                             const int e = q - REGCAP;
@@ -380,7 +384,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                                 if (x < oh) wmax = w > wmax ? w : wmax;                        \
                                 if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
                             }
-                            SVF_SLOT_SWITCH(kmax, SVF_BLOCK)
+                            SVF_SLOT_SWITCH(g4, SVF_BLOCK)
 #undef SVF_BLOCK
                             for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                 const int e = q - REGCAP;
@@ -407,7 +411,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             const uint32_t x = (uint32_t)f[k] - t1;                            \
                             if (x < oh) { B[k] += add + (uint32_t)f[k]; if (COUNT) cntU += 1; } \
                         }
-                        SVF_SLOT_SWITCH(kmax, SVF_UPDATE)
+                        SVF_SLOT_SWITCH(g4, SVF_UPDATE)
 #undef SVF_UPDATE
                         for (int q = REGCAP + tid; q < hw; q += THREADS) {
                             const int e = q - REGCAP;
