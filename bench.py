@@ -28,6 +28,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2606_22327_b200 import sharding as S  # noqa: E402
 from paper_2606_22327_b200 import traces as T  # noqa: E402
 
 METRIC = "simulated_request_steps_per_sec"
@@ -36,9 +37,19 @@ POLICIES = (0, 1, 2, 3)
 POLICY_NAMES = ("svf", "svf_1bit", "sjf", "fcfs")
 L2_FLUSH_BYTES = 512 << 20
 
-# algorithmic HBM bytes per request of the dominant kernel (k_sim): a, s, o read by
-# the validation pass (12) + rank and order (8) + start, finish (8) + latency word for p99 (8)
-SIM_BYTES_PER_REQUEST = 36
+# The dominant kernel (k_sim_slots, phase B) is bound by integer ALU issue, not by HBM (its state
+# is on chip).  Algorithmic work per launch = 4*E + 2*U lane-operations: E = running
+# entries examined over all head evaluations (two compares, one add, one max each), U = running
+# entries updated over all admissions (one compare, one add each); both counted exactly by the
+# kernel's counting variant on the same inputs.  Peak = the SM issue rate, from the guide's unit
+# counts: SMs x 4 schedulers x 32 lanes x 1 warp-instruction/cycle x max SM clock.
+OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
+# HBM bytes per request the same kernel must move: a, s, o (12) + rank (4) + (s, o, id, a) record
+# in priority order (16) + start, finish (8) + latency word for p99 (8)
+SIM_BYTES_PER_REQUEST = 48
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload, from the
+# `ncu --set full` capture summarised in profiles/r01_kslots_full.md
+SIM_DRAM_TRAFFIC_BYTES = 175.7e6
 
 
 def parse_args():
@@ -63,6 +74,19 @@ def measured_peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def alu_peak(torch, dev):
+    """Issue-rate roofline in lane-operations/s: SMs x 4 schedulers x 32 lanes x max SM clock."""
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    mhz, src = 1965.0, "B200_PROFILING.md max SM clock 1965 MHz"
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            mhz, src = float(json.load(open(p))["sm_max_mhz"]), "MEASURED_PEAKS.json sm_max_mhz"
+        except Exception:
+            pass
+    return sms * 4 * 32 * mhz * 1e6, f"{sms} SMs x 4 schedulers x 32 lanes x {mhz:g} MHz ({src})"
 
 
 class ClockSampler:
@@ -120,8 +144,8 @@ class ClockSampler:
 
 
 def make_batch(args, rank):
-    return T.config3(n_instances=args.instances, n=args.requests, lam=args.lam,
-                     first_instance=rank * args.instances)
+    lo, hi = S.weak_shard(rank, args.instances)        # per-GPU work fixed: weak scaling
+    return T.config3(n_instances=hi - lo, n=args.requests, lam=args.lam, first_instance=lo)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -281,29 +305,34 @@ def run_ours(args):
 
     # ---- reduce over ranks: max time, summed work -------------------------------------------
     decisions = sum(int(o.decisions.sum().item()) for o in outs)
-    if world > 1:
-        tmax = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tot = torch.tensor([rs_step, decisions, launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        total_ms, e2e_s = float(tmax[0]), float(tmax[1])
-        rs_all, dec_all, launches_all = float(tot[0]), float(tot[1]), int(tot[2])
-    else:
-        rs_all, dec_all, launches_all = float(rs_step), float(decisions), launches
+    (total_ms, e2e_s), (rs_all, dec_all, launches_all) = S.reduce_report(
+        [total_ms, e2e_s], [rs_step, decisions, launches], device=dev)   # max over ranks / summed
+    launches_all = int(launches_all)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
+    # ---- algorithmic work of the dominant kernel, counted by its counting variant (untimed) ----
+    B.set_profiling(2)
+    E = U = 0
+    for i, p in enumerate(POLICIES):
+        B.svf_simulate(dt_dev, p, out=outs[i], ws=ws)
+        e_, u_ = B.simulate_work_counts()
+        E += e_; U += u_
+    B.set_profiling(False)
+    ops_per_launch = (OPS_PER_EXAMINED * E + OPS_PER_UPDATED * U) / len(POLICIES)
+
     ms_per_step = total_ms / args.steps
     value = rs_all / (ms_per_step * 1e-3)
-    peak, peak_src = measured_peaks()
+    hbm_peak, hbm_src = measured_peaks()
+    peak_ops, peak_src = alu_peak(torch, dev)
     sim_bytes = SIM_BYTES_PER_REQUEST * batch.n_requests
-    achieved = sim_bytes / (sim_ms * 1e-3) / 1e9
+    achieved = ops_per_launch / (sim_ms * 1e-3)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "int32/int64", "data": "synthetic",
         "config": workload_config(args),
         "decisions_per_sec": dec_all / (ms_per_step * 1e-3),
         "requests_per_sec": world * batch.n_requests * len(POLICIES) / (ms_per_step * 1e-3),
@@ -312,13 +341,21 @@ def run_ours(args):
         "e2e": {"value": rs_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": 1e3 * e2e_s},
         "gpu_launches": launches_all,
-        "roofline": {"kernel": "k_sim (persistent simulator, phase B)", "bound": "hbm", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": sim_bytes,
+        "roofline": {"kernel": "k_sim_slots (persistent simulator, phase B)", "bound": "alu",
+                     "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "Tlane-op/s",
+                     "frac": achieved / peak_ops, "traffic": SIM_DRAM_TRAFFIC_BYTES,
+                     "peak_source": peak_src,
+                     "algorithmic_ops_per_launch": ops_per_launch,
+                     "entries_examined_per_launch": E / len(POLICIES),
+                     "entries_updated_per_launch": U / len(POLICIES),
                      "kernel_ms": sim_ms, "share_of_step": share,
-                     "note": "latency/issue bound by design: state stays on chip, HBM only sees the trace once "
-                             "(DESIGN.md 6); see 'kernels' for the HBM-bound pieces"},
+                     "hbm": {"algorithmic_bytes_per_launch": sim_bytes,
+                             "achieved_gbs": sim_bytes / (sim_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
+                             "frac": sim_bytes / (sim_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src},
+                     "note": "integer-ALU/issue bound by design: the per-step state stays in registers, HBM only "
+                             "sees the trace once (DESIGN.md 6); 'kernels' lists the HBM-bound pieces"},
     }
+    peak = hbm_peak
     if not args.no_extras:
         line["kernels"] = kernel_extras(B, torch, dev, peak)
         line["configs"] = config_extras(B, torch, dev)
@@ -368,8 +405,8 @@ def kernel_extras(B, torch, dev, peak):
     # admission decisions at depth (BASELINE.json configs[3] laws): W waiting, R running
     tr = T.config4(n=1 << 18)
     w = [torch.from_numpy(x).to(dev) for x in (tr.prompt, tr.output, tr.arrival, tr.bit)]
-    r_rem = torch.arange(1, 1025, dtype=torch.int32, device=dev) * 3
-    r_kv = torch.full((1024,), 600, dtype=torch.int32, device=dev)
+    r_rem = torch.arange(1, 1025, dtype=torch.int32, device=dev) * 2
+    r_kv = torch.full((1024,), 200, dtype=torch.int32, device=dev)
     res = B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem)
     wsa = torch.empty(B.svf_admit_workspace_bytes(1 << 18, 1024), dtype=torch.uint8, device=dev)
     ms = _time_cuda(torch, lambda: B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem, ws=wsa, out=res))
