@@ -39,14 +39,18 @@
 // its place at the head of the queue; the steps in between are counted into rounds/decisions
 // exactly as the step-by-step definition counts them (one blocked-head evaluation each).
 //
-// WAITING QUEUE: bitmap over ranks (keys are time-invariant, so the presort fixes the order):
-// one 32-bit word per lane in a register when the instance has at most 1024 requests (QREG),
-// else the two-level shared-memory bitmap of svf_state.cuh.  The two lowest waiting ranks with
-// their (s, o, id, a) are cached in registers: `head` and `second` (second's record is fetched
-// one admission ahead, hiding the L2 latency).  ARRIVALS come from a 32-wide register window
-// over (a, s, o, rank), refilled once per 32 arrivals; an arrival that becomes head/second
-// takes its record from the window.  OUTPUTS (start, finish, latency word) are buffered one
-// admission per lane and written 32 at a time.
+// WAITING QUEUE: bitmap over ranks (keys are time-invariant, so the presort fixes the order).
+//  * QREG (one warp per instance, at most 1024 requests): one 32-bit word per lane in a register,
+//    mirrored in shared memory where arrivals set their bits with one atomicOr each; the (s, o) of
+//    every waiting request sits in shared memory by rank (8 KB), written on arrival, so picking
+//    the next head never waits for global memory; id and arrival are only looked up when the
+//    outputs are written.
+//  * otherwise the two-level shared-memory bitmap of svf_state.cuh and (s, o, id, a) records in
+//    priority order in global memory.
+// The two lowest waiting ranks are cached in registers (`head`, `second`; second's record is
+// fetched one admission ahead).  ARRIVALS come from a 32-wide register window over
+// (a, s, o, rank), refilled once per 32 arrivals.  OUTPUTS (start, finish, latency word) are
+// buffered one admission per lane and written 32 at a time.
 #pragma once
 
 #include <limits.h>
@@ -116,6 +120,7 @@ struct SlotArgs {
     const uint8_t* bit;
     const int4* req;                 // [N] (s, o, id, a) at (instance offset + rank)
     const uint32_t* rank;            // [N] rank of (instance offset + local id)
+    const uint32_t* order;           // [N] local id at (instance offset + rank)
     int32_t *start, *finish;
     int64_t *tel, *peak, *rounds, *decisions;
     int32_t *makespan, *status;
@@ -132,6 +137,11 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
     const int nL0 = (qcap + 31) / 32, nL1 = (nL0 + 31) / 32;
     return align_up((size_t)nL0 * 4, 16) + align_up((size_t)nL1 * 4, 16) + 3 * align_up((size_t)ecap * 4, 16);
 }
+// QREG: shared memory holds the (s, o) records by rank and the bitmap mirror; the ext slots
+// (touched only when more than 32*K requests run at once) live in a global slot per CTA
+constexpr int QREG_RANKS = 1024;
+constexpr size_t QREG_SMEM_BYTES = (size_t)QREG_RANKS * 8 + 32 * 4;
+__host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
 
 // one reduction round over the group: a summed (mod 2^32), b maxed, c minned; uniform afterwards
 template <int THREADS>
@@ -155,24 +165,28 @@ __device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, 
     }
 }
 
-// straight-line code over register slots 4*g4-1 .. 0 (g4 = groups of four slots in use): one
-// indexed branch, no loop overhead; four slots per basic block so that the compiler can
-// interleave their dependent chains (x -> compare -> predicated op).  A slot past the high-water
-// mark is dead (f = 0) and costs its instructions only.
-#define SVF_SLOT_SWITCH(g4, OP)                                                               \
-    switch (g4) {                                                                             \
-    default:                                                                                  \
-    case 4: OP(15) OP(14) OP(13) OP(12)                                                       \
-    case 3: OP(11) OP(10) OP(9)  OP(8)                                                        \
-    case 2: OP(7)  OP(6)  OP(5)  OP(4)                                                        \
-    case 1: OP(3)  OP(2)  OP(1)  OP(0)                                                        \
-    case 0: break;                                                                            \
-    }
+
+// straight-line code over register slots 4*g4-1 .. 0 (g4 = groups of four slots in use): at most
+// four uniform compare-and-branch, no indexed branch, no loop overhead; four slots per basic
+// block so that the compiler can interleave their dependent chains (x -> compare -> predicated
+// op).  A slot past the high-water mark is dead (f = 0) and costs its instructions only.
+#define SVF_SLOT_GROUPS(g4, OP)                                                               \
+    if ((g4) >= 4) { OP(15) OP(14) OP(13) OP(12) }                                            \
+    if ((g4) >= 3) { OP(11) OP(10) OP(9)  OP(8)  }                                            \
+    if ((g4) >= 2) { OP(7)  OP(6)  OP(5)  OP(4)  }                                            \
+    if ((g4) >= 1) { OP(3)  OP(2)  OP(1)  OP(0)  }
+
+// write into register slot ik (uniform) of the owning thread: a tree of uniform branches
+#define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
+#define SVF_PUT4(ik, OP, k0)  if ((ik) & 2) { SVF_PUT2(ik, OP, k0 + 2) } else { SVF_PUT2(ik, OP, k0) }
+#define SVF_PUT8(ik, OP, k0)  if ((ik) & 4) { SVF_PUT4(ik, OP, k0 + 4) } else { SVF_PUT4(ik, OP, k0) }
+#define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
 
 template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
 __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
 {
-    static_assert(K == 16, "SVF_SLOT_SWITCH is written out for 16 register slots per thread");
+    static_assert(K == 16, "SVF_SLOT_GROUPS / SVF_PUT16 are written out for 16 register slots per thread");
+    static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
     using G = Group<THREADS>;
     constexpr int WARPS = THREADS / 32;
     constexpr int REGCAP = THREADS * K;
@@ -185,7 +199,9 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     int parity = 0, rparity = 0;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
 
-    char* sbase = SMEM ? dyn_smem : g.gstate + (size_t)blockIdx.x * g.slot_bytes;
+    // state placement: QREG: records + bitmap mirror in shared memory, ext slots in the global
+    // slot; else bitmaps + ext slots together in shared memory (SMEM) or in the global slot
+    char* sbase = (SMEM && !QREG) ? dyn_smem : g.gstate + (size_t)blockIdx.x * g.slot_bytes;
     const int capL0 = QREG ? 0 : (g.qcap + 31) / 32, capL1 = (capL0 + 31) / 32;
     uint32_t* L0 = reinterpret_cast<uint32_t*>(sbase);
     uint32_t* L1 = reinterpret_cast<uint32_t*>(sbase + align_up((size_t)capL0 * 4, 16));
@@ -194,6 +210,8 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     int32_t* ef = reinterpret_cast<int32_t*>(ebase);
     uint32_t* eB = reinterpret_cast<uint32_t*>(ebase + estride);
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
+    int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
+    uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QREG_RANKS * 8);  // QREG only
     const int Mi = (int)g.M;
     const bool want_start = g.start != nullptr, want_finish = g.finish != nullptr, want_latw = g.latw != nullptr;
 
@@ -208,7 +226,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         const int64_t n64 = g.off[j + 1] - base;
         uint32_t flags = 0;
         if (n64 < 0 || n64 > g.max_instance || base < 0 || base + (n64 > 0 ? n64 : 0) > g.N ||
-            g.off[0] != 0 || g.off[g.I] != g.N)
+            g.off[0] != 0 || g.off[g.I] != g.N || (QREG && n64 > QREG_RANKS))
             flags |= F_LAYOUT;
         const int n = (flags & F_LAYOUT) ? 0 : (int)n64;
         const int32_t* __restrict__ a = g.a + base;
@@ -247,6 +265,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             }
         } else {
             const uint32_t* __restrict__ rnk = g.rank + base;
+            const uint32_t* __restrict__ ord = g.order + base;
             const int4* __restrict__ req = g.req + base;
             int32_t* __restrict__ out_start = g.start + base;
             int32_t* __restrict__ out_finish = g.finish + base;
@@ -254,7 +273,9 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             const uint64_t jhi = (uint64_t)j << 32;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
             uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32)
-            if (!QREG) {
+            if (QREG) {
+                qbits[lane] = 0;
+            } else {
                 for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
                 for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
             }
@@ -277,17 +298,20 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
             };
             // output buffer: admission number m sits in lane m % 32 of warp 0 until 32 are there
+            // (QREG: b_id holds the RANK; id and arrival are looked up when the buffer is written)
             int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
             auto flush = [&](int count) {
                 if (wrp == 0 && lane < count) {
-                    if (want_start) out_start[b_id] = b_t;
-                    if (want_finish) out_finish[b_id] = b_f;
-                    if (want_latw) out_latw[b_id] = jhi | (uint32_t)b_lat;
-                    tel += b_lat;
+                    int id = b_id, lat = b_lat;
+                    if (QREG) { id = (int)ord[b_id]; lat = b_f - a[id]; }
+                    if (want_start) out_start[id] = b_t;
+                    if (want_finish) out_finish[id] = b_f;
+                    if (want_latw) out_latw[id] = jhi | (uint32_t)lat;
+                    tel += lat;
                     mk = b_f > mk ? b_f : mk;
                 }
             };
-            if (!QREG) G::sync();
+            G::sync();
 
             Rec head, second;
             head.r = INT_MAX; head.s = head.o = head.id = head.a = 0;
@@ -306,38 +330,56 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                     const uint32_t m = __ballot_sync(FULL, v);
                     if (!m) break;
                     if (QREG) {
-                        for (uint32_t mm = m; mm; mm &= mm - 1u) {
-                            const int r = __shfl_sync(FULL, rw, __ffs(mm) - 1);
-                            if (lane == (r >> 5)) qword |= 1u << (r & 31);
-                        }
+                        // the owner's plain store of a cleared word comes before these atomics
+                        if (!arrived) __syncwarp();
+                        if (v) { qrec[rw] = make_int2(sw, ow); atomicOr(&qbits[rw >> 5], 1u << (rw & 31)); }
                     } else {
                         // nobody may still be reading the bitmap for the previous step
                         if (!arrived) G::sync();
                         if (wrp == 0 && v) queue_set(L0, L1, rw);
-                    }
-                    arrived = true;
-                    const int r1 = __reduce_min_sync(FULL, v ? rw : INT_MAX);
-                    if (r1 < second.r) {
-                        const int l1 = __ffs(__ballot_sync(FULL, v && rw == r1)) - 1;
-                        if (r1 < head.r) {
-                            const int r2 = __reduce_min_sync(FULL, (v && lane != l1) ? rw : INT_MAX);
-                            const Rec n1 = win_rec(l1, r1);
-                            if (r2 < head.r) {
-                                const int l2 = __ffs(__ballot_sync(FULL, v && lane != l1 && rw == r2)) - 1;
-                                second = win_rec(l2, r2);
+                        const int r1 = __reduce_min_sync(FULL, v ? rw : INT_MAX);
+                        if (r1 < second.r) {
+                            const int l1 = __ffs(__ballot_sync(FULL, v && rw == r1)) - 1;
+                            if (r1 < head.r) {
+                                const int r2 = __reduce_min_sync(FULL, (v && lane != l1) ? rw : INT_MAX);
+                                const Rec n1 = win_rec(l1, r1);
+                                if (r2 < head.r) {
+                                    const int l2 = __ffs(__ballot_sync(FULL, v && lane != l1 && rw == r2)) - 1;
+                                    second = win_rec(l2, r2);
+                                } else {
+                                    second = head;
+                                }
+                                head = n1;
+                                t_lb = t;                 // a new head: evaluate it now
                             } else {
-                                second = head;
+                                second = win_rec(l1, r1);
                             }
-                            head = n1;
-                            t_lb = t;                 // a new head: evaluate it now
-                        } else {
-                            second = win_rec(l1, r1);
                         }
                     }
+                    arrived = true;
                     next += __popc(m);
                     if (next < wb + 32) break;
                 }
-                if (!QREG && arrived && THREADS == 32) __syncwarp();
+                if (arrived) {
+                    if (QREG) {
+                        // reload the bitmap word and take head and second from it
+                        __syncwarp();
+                        qword = qbits[lane];
+                        const int r0 = qreg_first_ge(qword, 0);
+                        if (r0 != head.r) {
+                            const int2 v = qrec[r0];
+                            head.r = r0; head.s = v.x; head.o = v.y;
+                            t_lb = t;                     // a new head: evaluate it now
+                        }
+                        const int r1 = qreg_first_ge(qword, r0 + 1);
+                        if (r1 != second.r) {
+                            second.r = r1;
+                            if (r1 != INT_MAX) { const int2 v = qrec[r1]; second.s = v.x; second.o = v.y; }
+                        }
+                    } else if (THREADS == 32) {
+                        __syncwarp();
+                    }
+                }
 
                 // 3. ADMIT
                 if (head.r != INT_MAX) {
@@ -351,26 +393,29 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                         int viol = INT_MIN;
                         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
                         const int g4 = (kmax + 3) >> 2;
+                        const bool use_ext = hw > REGCAP;
 #define SVF_EVAL(k) {                                                                          \
                             const uint32_t x = (uint32_t)f[k] - t1;                            \
                             if (f[k] >= fh) acc += c[k] + fhu;                                 \
-                            if (x < oh) viol = __viaddmax_s32((int)B[k], (int)Kc, viol);            \
+                            if (x < oh) viol = __viaddmax_s32((int)B[k], (int)Kc, viol);       \
                             dm = __funnelshift_l(x, dm, 1);                                    \
                             if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
                         }
-                        SVF_SLOT_SWITCH(g4, SVF_EVAL)
+                        SVF_SLOT_GROUPS(g4, SVF_EVAL)
 #undef SVF_EVAL
                         // lowest free register slot of this thread: bit k of dm = slot k is dead
                         const int kfree = dm ? __ffs(dm) - 1 : 4 * g4;
                         int fidx = kfree < K ? (kfree << TSHIFT) + tid : INT_MAX;
-                        for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                            const int e = q - REGCAP;
-                            const int fk = ef[e];
-                            const uint32_t x = (uint32_t)fk - t1;
-                            if (fk >= fh) acc += ec[e] + fhu;
-                            if (x < oh) viol = __viaddmax_s32((int)eB[e], (int)Kc, viol);
-                            if (x >> 31) fidx = fidx < q ? fidx : q;
-                            if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
+                        if (use_ext) {
+                            for (int q = REGCAP + tid; q < hw; q += THREADS) {
+                                const int e = q - REGCAP;
+                                const int fk = ef[e];
+                                const uint32_t x = (uint32_t)fk - t1;
+                                if (fk >= fh) acc += ec[e] + fhu;
+                                if (x < oh) viol = __viaddmax_s32((int)eB[e], (int)Kc, viol);
+                                if (x >> 31) fidx = fidx < q ? fidx : q;
+                                if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
+                            }
                         }
                         reduce_add_max_min<THREADS>(acc, viol, fidx, red, rparity);
                         const int Ah = head.s + head.o + (int)acc;        // exact: 0 <= A_h <= 2M < 2^31
@@ -379,21 +424,23 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             int wmax = 0, minge = INT_MAX;
 #define SVF_BLOCK(k) {                                                                         \
                                 const uint32_t x = (uint32_t)f[k] - t1;                        \
-                                const int v = (int)(B[k] + Kc), d = (int)x + 1;                  \
+                                const int v = (int)(B[k] + Kc), d = (int)x + 1;                \
                                 const int w = v < d ? v : d;                                   \
                                 if (x < oh) wmax = w > wmax ? w : wmax;                        \
                                 if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
                             }
-                            SVF_SLOT_SWITCH(g4, SVF_BLOCK)
+                            SVF_SLOT_GROUPS(g4, SVF_BLOCK)
 #undef SVF_BLOCK
-                            for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                                const int e = q - REGCAP;
-                                const int fk = ef[e];
-                                const uint32_t x = (uint32_t)fk - t1;
-                                const int v = (int)(eB[e] + Kc), d = (int)x + 1;
-                                const int w = v < d ? v : d;
-                                if (x < oh) wmax = w > wmax ? w : wmax;
-                                if (fk >= fh) minge = fk < minge ? fk : minge;
+                            if (use_ext) {
+                                for (int q = REGCAP + tid; q < hw; q += THREADS) {
+                                    const int e = q - REGCAP;
+                                    const int fk = ef[e];
+                                    const uint32_t x = (uint32_t)fk - t1;
+                                    const int v = (int)(eB[e] + Kc), d = (int)x + 1;
+                                    const int w = v < d ? v : d;
+                                    if (x < oh) wmax = w > wmax ? w : wmax;
+                                    if (fk >= fh) minge = fk < minge ? fk : minge;
+                                }
                             }
                             uint32_t z = 0;
                             reduce_add_max_min<THREADS>(z, wmax, minge, red, rparity);
@@ -411,22 +458,20 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             const uint32_t x = (uint32_t)f[k] - t1;                            \
                             if (x < oh) { B[k] += add + (uint32_t)f[k]; if (COUNT) cntU += 1; } \
                         }
-                        SVF_SLOT_SWITCH(g4, SVF_UPDATE)
+                        SVF_SLOT_GROUPS(g4, SVF_UPDATE)
 #undef SVF_UPDATE
-                        for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                            const int e = q - REGCAP;
-                            const int fk = ef[e];
-                            if ((uint32_t)fk - t1 < oh) { eB[e] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
+                        if (use_ext) {
+                            for (int q = REGCAP + tid; q < hw; q += THREADS) {
+                                const int e = q - REGCAP;
+                                const int fk = ef[e];
+                                if ((uint32_t)fk - t1 < oh) { eB[e] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
+                            }
                         }
                         if (idx < REGCAP) {
                             const bool mine = (idx & (THREADS - 1)) == tid;
-#define SVF_PUT(k) { if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; } break; }
-                            switch (idx >> TSHIFT) {
-                            case 0: SVF_PUT(0) case 1: SVF_PUT(1) case 2: SVF_PUT(2) case 3: SVF_PUT(3)
-                            case 4: SVF_PUT(4) case 5: SVF_PUT(5) case 6: SVF_PUT(6) case 7: SVF_PUT(7)
-                            case 8: SVF_PUT(8) case 9: SVF_PUT(9) case 10: SVF_PUT(10) case 11: SVF_PUT(11)
-                            case 12: SVF_PUT(12) case 13: SVF_PUT(13) case 14: SVF_PUT(14) default: SVF_PUT(15)
-                            }
+                            const int ik = idx >> TSHIFT;
+#define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
+                            SVF_PUT16(ik, SVF_PUT)
 #undef SVF_PUT
                         } else if (((idx - REGCAP) & (THREADS - 1)) == tid) {
                             const int e = idx - REGCAP;
@@ -438,20 +483,29 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             const int p2 = Ah > pj ? Ah : pj;
                             peak = p2 > peak ? p2 : peak;
                         }
-                        if (QREG) { if (lane == (head.r >> 5)) qword &= ~(1u << (head.r & 31)); }
-                        else if (tid == 0) queue_clear(L0, L1, head.r);
-                        if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
+                        if (QREG) {
+                            if (lane == (head.r >> 5)) { qword &= ~(1u << (head.r & 31)); qbits[lane] = qword; }
+                            if (lane == (started & 31)) { b_id = head.r; b_t = t; b_f = fh; }
+                        } else {
+                            if (tid == 0) queue_clear(L0, L1, head.r);
+                            if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
+                        }
                         ++started; ++decisions;
                         if ((started & 31) == 0) flush(32);
                         // promote the second; fetch the record behind it one admission ahead
                         head = second;
                         second.r = INT_MAX;
                         if (head.r == INT_MAX) break;
-                        const int r = QREG ? qreg_first_ge(qword, head.r + 1)
-                                           : queue_first_ge(L0, L1, n, nL1, head.r + 1);
-                        if (r != INT_MAX) {
-                            const int4 qv = req[r];
-                            second.r = r; second.s = qv.x; second.o = qv.y; second.id = qv.z; second.a = qv.w;
+                        if (QREG) {
+                            const int r = qreg_first_ge(qword, head.r + 1);
+                            second.r = r;
+                            if (r != INT_MAX) { const int2 v = qrec[r]; second.s = v.x; second.o = v.y; }
+                        } else {
+                            const int r = queue_first_ge(L0, L1, n, nL1, head.r + 1);
+                            if (r != INT_MAX) {
+                                const int4 qv = req[r];
+                                second.r = r; second.s = qv.x; second.o = qv.y; second.id = qv.z; second.a = qv.w;
+                            }
                         }
                     }
                     if (head.r != INT_MAX) ++decisions;          // one blocked-head evaluation (R16)

@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(256) k_sim_rank(SimArgs g, const SortPlan* __r
         if (r >= 0 && base + seq < g.N) {
             rank[base + seq] = (uint32_t)r;
             const int64_t i = base + seq;
-            g.req[p] = make_int4(__ldg(g.s + i), __ldg(g.o + i), (int)seq, __ldg(g.a + i));
+            if (g.req) g.req[p] = make_int4(__ldg(g.s + i), __ldg(g.o + i), (int)seq, __ldg(g.a + i));
         }
     }
 }
@@ -298,6 +298,8 @@ struct SimConfig {
     int ecap, qcap;         // slots kernel: ext slots per instance, bitmap capacity
     bool qreg;              // slots kernel: waiting bitmap in one register per lane (<= 1024 ranks)
     size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
+    size_t gslot_bytes;     // bytes of the per-CTA slot in global memory (0: none)
+    int max_cta_per_sm;     // bound on resident CTAs per SM (sizes the global slots)
     int threads;
     bool smem;
     int cap;
@@ -330,17 +332,29 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M)
     while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
     if (threads == 64) threads = 128;
     if (threads == 512) threads = 1024;
+    c.gslot_bytes = 0; c.max_cta_per_sm = 2;
     if (c.slots) {
         auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
-        c.qreg = mx <= 1024;
-        if (c.qreg) c.qcap = 0;
-        if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) threads = 128;
-        c.ecap = ext_of(threads);
-        c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
-        c.smem = c.qreg || c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
+        c.qreg = threads == 32 && mx <= QREG_RANKS;
+        if (c.qreg) {
+            // records + bitmap mirror in shared memory, ext slots in a global slot per CTA
+            c.qcap = 0;
+            c.ecap = ext_of(32);
+            c.state_bytes = QREG_SMEM_BYTES;
+            c.smem = true;
+            c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
+            c.max_cta_per_sm = 32;
+        } else {
+            if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) threads = 128;
+            c.ecap = ext_of(threads);
+            c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
+            c.smem = c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
+            if (!c.smem) c.gslot_bytes = align_up(c.state_bytes, 256);
+        }
     } else {
         c.state_bytes = state_bytes(c.cap);
         c.smem = c.state_bytes <= SMEM_STATE_LIMIT;
+        if (!c.smem) c.gslot_bytes = align_up(c.state_bytes, 256);
     }
     c.dyn_smem = c.smem ? c.state_bytes : 0;
     c.threads = threads;
@@ -379,13 +393,7 @@ int slots_grid(const SimConfig& c, int64_t I)
 int sim_grid_any(const SimConfig& c, int64_t I)
 {
     if (c.slots) {
-        if (c.qreg) {
-            switch (c.threads) {
-            case 32: return slots_grid<32, true, true>(c, I);
-            case 128: return slots_grid<128, true, true>(c, I);
-            default: return slots_grid<256, true, true>(c, I);
-            }
-        }
+        if (c.qreg) return slots_grid<32, true, true>(c, I);
         if (c.smem) {
             switch (c.threads) {
             case 32: return slots_grid<32, true, false>(c, I);
@@ -435,7 +443,7 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
     w->counts = (unsigned long long*)(base + p); p += 256;
     w->status_tmp = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
     w->work_ctr = (unsigned long long*)(base + p); p += 256;
-    w->slot_bytes = c.smem ? 0 : align_up(c.state_bytes, 256);
+    w->slot_bytes = c.gslot_bytes;
     w->grid_slots = grid_slots;
     w->gstate = base + p; p += w->slot_bytes * (size_t)grid_slots;
     w->total = p;
@@ -473,7 +481,9 @@ extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr)
     for (int64_t M : {(int64_t)0, (int64_t)1 << 30}) {
         SimConfig c = sim_config(tr, M);
         SimWs w;
-        sim_ws_layout(&w, nullptr, tr, c, c.smem ? 0 : 2 * sm_count());
+        int64_t slots = c.gslot_bytes ? (int64_t)c.max_cta_per_sm * sm_count() : 0;
+        if (slots > tr->n_instances) slots = tr->n_instances;
+        sim_ws_layout(&w, nullptr, tr, c, (int)slots);
         need = w.total > need ? w.total : need;
     }
     return need + 256;
@@ -501,16 +511,16 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
     const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
     int grid = sim_grid_any(c, I);
-    if (!c.smem && grid > 2 * sm_count()) grid = 2 * sm_count();
+    if (c.gslot_bytes && grid > c.max_cta_per_sm * sm_count()) grid = c.max_cta_per_sm * sm_count();
     SimWs w;
-    sim_ws_layout(&w, base, tr, c, c.smem ? 0 : grid);
+    sim_ws_layout(&w, base, tr, c, c.gslot_bytes ? grid : 0);
     if (w.total > avail) return SVF_EWORKSPACE;
 
     SimArgs g;
     g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
     g.policy = policy; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
     g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
-    g.order = w.order; g.rank = w.rank; g.req = w.req;
+    g.order = w.order; g.rank = w.rank; g.req = (c.slots && c.qreg) ? nullptr : w.req;
     g.start = out->start; g.finish = out->finish; g.tel = out->total_latency; g.peak = out->peak_kv;
     g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
     g.status = out->status ? out->status : w.status_tmp;
@@ -538,7 +548,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         q.I = I; q.N = N; q.M = M; q.max_instance = tr->max_instance;
         q.policy = policy; q.O0 = tr->O0; q.O1 = tr->O1;
         q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
-        q.req = w.req; q.rank = w.rank;
+        q.req = w.req; q.rank = w.rank; q.order = w.order;
         q.start = g.start; q.finish = g.finish; q.tel = g.tel; q.peak = g.peak; q.rounds = g.rounds;
         q.decisions = g.decisions; q.makespan = g.makespan; q.status = g.status; q.latw = g.latw;
         q.work_ctr = w.work_ctr; q.work_counts = w.counts;
@@ -554,11 +564,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
             else       k_sim_slots<T, SLOT_K, S, false, Q><<<grid, T, c.dyn_smem, st>>>(q);   \
         } while (0)
         if (c.qreg) {
-            switch (c.threads) {
-            case 32: SVF_SLOTS_LAUNCH(32, true, true); break;
-            case 128: SVF_SLOTS_LAUNCH(128, true, true); break;
-            default: SVF_SLOTS_LAUNCH(256, true, true); break;
-            }
+            SVF_SLOTS_LAUNCH(32, true, true);
         } else if (c.smem) {
             switch (c.threads) {
             case 32: SVF_SLOTS_LAUNCH(32, true, false); break;
