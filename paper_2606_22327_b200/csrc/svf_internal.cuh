@@ -86,6 +86,14 @@ void   sort_ws_carve(SortWs* w, void* base, int64_t n, int bit_lo, int bit_hi);
 // Returns a cudaError_t as int; adds the number of launches to *launches.
 int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int64_t n, int bit_lo,
              int bit_hi, cudaStream_t st, int64_t* launches);
+// Segmented sort of small segments in shared memory (one CTA per instance, max_instance <=
+// SEG_SORT_MAX): computes the priority keys from the trace and writes order[] (local id at
+// instance offset + rank), rank[] (rank of instance offset + local id) and, if req != nullptr,
+// the (s, o, id, a) records in priority order.  One launch.
+constexpr int SEG_SORT_MAX = 4096;
+int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
+                  const int32_t* s, const int32_t* o, const int32_t* a, const uint8_t* bit, int32_t O0,
+                  int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st, int64_t* launches);
 // copy plan->result to out unless it already is out
 int sort_result_to(const SortWs& w, uint64_t* out, int64_t n, cudaStream_t st, int64_t* launches);
 

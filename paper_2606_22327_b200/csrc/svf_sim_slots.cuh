@@ -50,7 +50,8 @@
 // The two lowest waiting ranks are cached in registers (`head`, `second`; second's record is
 // fetched one admission ahead).  ARRIVALS come from a 32-wide register window over
 // (a, s, o, rank), refilled once per 32 arrivals.  OUTPUTS (start, finish, latency word) are
-// buffered one admission per lane and written 32 at a time.
+// buffered one admission per lane and written 32 at a time; p99 (nearest rank) is a radix selection
+// over the instance's latencies by the same thread group at the end of the instance.
 #pragma once
 
 #include <limits.h>
@@ -124,7 +125,8 @@ struct SlotArgs {
     int32_t *start, *finish;
     int64_t *tel, *peak, *rounds, *decisions;
     int32_t *makespan, *status;
-    uint64_t* latw;
+    uint32_t* lat;                   // [N] latency of (instance offset + local id): scratch of the p99 selection
+    int64_t* p99;                    // [I] or NULL
     unsigned long long* work_ctr;
     unsigned long long* work_counts; // [2] E, U (only written by the COUNT variant)
     char* gstate; size_t slot_bytes; // per-CTA state when it does not fit in shared memory
@@ -166,6 +168,56 @@ __device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, 
 }
 
 
+// k-th smallest (k >= 1) of v[0..n) by MSB-first radix selection, all threads of the group, result
+// uniform.  One 256-bin histogram in shared memory per significant byte; v was written by this
+// group before a barrier (read with ld.cg, never through the non-coherent path).
+template <int THREADS>
+__device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, int k, uint32_t* hist,
+                                                     int (*scratch)[64], int& parity)
+{
+    using G = Group<THREADS>;
+    const int tid = threadIdx.x, lane = tid & 31;
+    uint32_t vor = 0;
+    for (int i = tid; i < n; i += THREADS) vor |= __ldcg(v + i);
+    vor = G::or_u32(vor, scratch, parity);
+    uint32_t prefix = 0, pmask = 0;
+    for (int shift = vor ? ((31 - __clz(vor)) & ~7) : 0; shift >= 0; shift -= 8) {
+        for (int i = tid; i < 256; i += THREADS) hist[i] = 0;
+        G::sync();
+        for (int i = tid; i < n; i += THREADS) {
+            const uint32_t x = __ldcg(v + i);
+            if ((x & pmask) == prefix) atomicAdd(&hist[(x >> shift) & 255u], 1u);
+        }
+        G::sync();
+        // every warp redundantly: lane l owns digits 8l .. 8l+7
+        uint32_t c[8], s8 = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { c[q] = hist[lane * 8 + q]; s8 += c[q]; }
+        uint32_t inc = s8;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t u = __shfl_up_sync(FULL, inc, d); if (lane >= d) inc += u; }
+        const uint32_t b = __ballot_sync(FULL, inc >= (uint32_t)k);
+        const int L = b ? __ffs(b) - 1 : 31;
+        const int kk = k - (int)__shfl_sync(FULL, inc - s8, L);
+        int d = 7; uint32_t cum = 0;
+        {
+            uint32_t run = 0; bool found = false;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                if (!found && run + c[q] >= (uint32_t)kk) { d = q; cum = run; found = true; }
+                run += c[q];
+            }
+        }
+        d = __shfl_sync(FULL, d, L);
+        cum = __shfl_sync(FULL, cum, L);
+        k = kk - (int)cum;
+        prefix |= (uint32_t)(L * 8 + d) << shift;
+        pmask |= 255u << shift;
+        G::sync();
+    }
+    return prefix;
+}
+
 // straight-line code over register slots 4*g4-1 .. 0 (g4 = groups of four slots in use): at most
 // four uniform compare-and-branch, no indexed branch, no loop overhead; four slots per basic
 // block so that the compiler can interleave their dependent chains (x -> compare -> predicated
@@ -196,6 +248,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     __shared__ int scratch[2][64];
     __shared__ int red[2][WARPS][3];
     __shared__ long long inst_s;
+    __shared__ uint32_t hist[256];
     int parity = 0, rparity = 0;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
 
@@ -213,7 +266,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
     uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QREG_RANKS * 8);  // QREG only
     const int Mi = (int)g.M;
-    const bool want_start = g.start != nullptr, want_finish = g.finish != nullptr, want_latw = g.latw != nullptr;
+    const bool want_start = g.start != nullptr, want_finish = g.finish != nullptr, want_p99 = g.p99 != nullptr;
 
     while (true) {
         if (tid == 0) inst_s = (long long)atomicAdd(g.work_ctr, 1ull);
@@ -256,12 +309,12 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         int mk = 0, peak = 0;
         uint32_t rounds = 0, decisions = 0;
         long long cntE = 0, cntU = 0;
+        int64_t p99v = 0;
 
         if (status != SVF_OK || n == 0) {
             for (int i = tid; i < n; i += THREADS) {
                 if (want_start) g.start[base + i] = -1;
                 if (want_finish) g.finish[base + i] = -1;
-                if (want_latw) g.latw[base + i] = (uint64_t)j << 32;
             }
         } else {
             const uint32_t* __restrict__ rnk = g.rank + base;
@@ -269,8 +322,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             const int4* __restrict__ req = g.req + base;
             int32_t* __restrict__ out_start = g.start + base;
             int32_t* __restrict__ out_finish = g.finish + base;
-            uint64_t* __restrict__ out_latw = g.latw + base;
-            const uint64_t jhi = (uint64_t)j << 32;
+            uint32_t* out_lat = g.lat + base;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
             uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32)
             if (QREG) {
@@ -306,7 +358,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                     if (QREG) { id = (int)ord[b_id]; lat = b_f - a[id]; }
                     if (want_start) out_start[id] = b_t;
                     if (want_finish) out_finish[id] = b_f;
-                    if (want_latw) out_latw[id] = jhi | (uint32_t)lat;
+                    if (want_p99) out_lat[id] = (uint32_t)lat;
                     tel += lat;
                     mk = b_f > mk ? b_f : mk;
                 }
@@ -525,6 +577,10 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 t = tn;
             }
             flush(started & 31);
+            if (want_p99) {                       // nearest rank ceil(0.99 n), 1-based (R13)
+                G::sync();
+                p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity);
+            }
         }
         if (COUNT) {
 #pragma unroll
@@ -542,6 +598,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         if (tid == 0) {
             if (g.tel) g.tel[j] = tel;
             if (g.peak) g.peak[j] = (int64_t)peak;
+            if (g.p99) g.p99[j] = p99v;
             if (g.rounds) g.rounds[j] = (int64_t)rounds;
             if (g.decisions) g.decisions[j] = (int64_t)decisions;
             if (g.makespan) g.makespan[j] = mk;

@@ -531,7 +531,12 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     prof_mark(0, st);
     if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
     int rc = 0;
-    if (N > 0) {
+    if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
+        // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance
+        rc = seg_sort_keys(policy, I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->arrival,
+                           tr->bit, tr->O0, tr->O1, w.order, w.rank, g.req, st, &g_launches_sim);
+        if (rc) return SVF_ECUDA;
+    } else if (N > 0) {
         int64_t blocks = ceil_div(N, 256);
         const int64_t capb = (int64_t)sm_count() * 8;
         if (blocks > capb) blocks = capb;
@@ -550,7 +555,8 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
         q.req = w.req; q.rank = w.rank; q.order = w.order;
         q.start = g.start; q.finish = g.finish; q.tel = g.tel; q.peak = g.peak; q.rounds = g.rounds;
-        q.decisions = g.decisions; q.makespan = g.makespan; q.status = g.status; q.latw = g.latw;
+        q.decisions = g.decisions; q.makespan = g.makespan; q.status = g.status;
+        q.lat = reinterpret_cast<uint32_t*>(w.words0); q.p99 = out->p99_latency;   // p99 selected in the kernel
         q.work_ctr = w.work_ctr; q.work_counts = w.counts;
         q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
         const bool count = g_profiling == 2;
@@ -602,7 +608,7 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
     if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
     prof_mark(2, st);
 
-    if (out->p99_latency) {
+    if (out->p99_latency && !c.slots) {
         if (N > 0) {
             rc = sort_u64(w.sort, w.words0, w.words1, w.words0, N, 0, 32 + c.ib, st, &g_launches_sim);
             if (rc) return SVF_ECUDA;

@@ -261,6 +261,125 @@ __global__ void k_sort_copy_result(const SortPlan* __restrict__ plan, uint64_t* 
 
 __global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan->result = in; }
 
+// ---- segmented sort of SMALL segments, entirely in shared memory ------------------------------
+// One CTA per instance (svf_simulate's presort when every instance has at most SEG_SORT_MAX
+// requests): keys (Eq. 1 / Eq. 2 / o / a) are computed from the trace, packed as (key << 32) + id,
+// sorted by stable LSD radix passes over the significant key bytes only (an OR-reduction of the
+// keys tells how many), ping-pong between two shared-memory buffers with the same warp-ballot
+// ranking as k_sort_pass, and the priority order leaves the chip once: order[] (id at rank),
+// rank[] (rank of id) and, if wanted, the (s, o, id, a) records in priority order.  HBM traffic:
+// 12-13 B read + 8 B (24 B with records) written per request, against 8 + 16 B per executed pass
+// of the device-wide sort.
+template <int THREADS>
+__device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out, int n, int ipt,
+                                         int shift, uint32_t* whist, uint32_t* toff_s, uint32_t* warp_tot)
+{
+    constexpr int WARPS = THREADS / 32;
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    for (int i = tid; i < WARPS * SORT_RADIX; i += THREADS) whist[i] = 0;
+    __syncthreads();
+    const int wbase = wrp * 32 * ipt;
+    uint32_t* wh = whist + wrp * SORT_RADIX;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    uint64_t key[SORT_IPT];
+    uint32_t rank[SORT_IPT];
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        if (i >= ipt) break;                                   // uniform
+        const int e = wbase + i * 32 + lane;
+        const bool valid = e < n;
+        key[i] = valid ? in[e] : 0ull;
+        const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & 0xffu) : SORT_RADIX;
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t base = 0;
+        if (valid) base = wh[d];
+        __syncwarp();
+        if (valid && lane == (31 - __clz(peers))) wh[d] = base + __popc(peers);
+        __syncwarp();
+        rank[i] = base + __popc(peers & lt_mask);
+    }
+    __syncthreads();
+    // digit d (threads 0..255): exclusive scan over warps, then over digits
+    uint32_t count = 0;
+    if (tid < SORT_RADIX) {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) { uint32_t c = whist[w * SORT_RADIX + tid]; whist[w * SORT_RADIX + tid] = run; run += c; }
+        count = run;
+    }
+    uint32_t inc = count;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+    if (lane == 31) warp_tot[wrp] = inc;
+    __syncthreads();
+    if (tid < SORT_RADIX) {
+        uint32_t off = 0;
+        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
+        toff_s[tid] = off + inc - count;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        if (i >= ipt) break;
+        if (wbase + i * 32 + lane < n) {
+            const uint32_t d = (uint32_t)(key[i] >> shift) & 0xffu;
+            out[toff_s[d] + wh[d] + rank[i]] = key[i];
+        }
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I, int64_t N, int cap,
+                                                           const int64_t* __restrict__ off,
+                                                           const int32_t* __restrict__ s, const int32_t* __restrict__ o,
+                                                           const int32_t* __restrict__ a, const uint8_t* __restrict__ bit,
+                                                           int32_t O0, int32_t O1, uint32_t* __restrict__ order,
+                                                           uint32_t* __restrict__ rank, int4* __restrict__ req)
+{
+    static_assert(SORT_THREADS == SORT_RADIX, "one thread per digit in the scans");
+    constexpr int WARPS = SORT_THREADS / 32;
+    extern __shared__ __align__(16) uint64_t seg_buf[];       // [2][cap]
+    __shared__ uint32_t whist[WARPS * SORT_RADIX];
+    __shared__ uint32_t toff_s[SORT_RADIX];
+    __shared__ uint32_t warp_tot[WARPS];
+    __shared__ uint32_t kor_s;
+    const int tid = threadIdx.x;
+    for (int64_t j = blockIdx.x; j < I; j += gridDim.x) {
+        const int64_t base = off[j], n64 = off[j + 1] - base;
+        if (n64 <= 0 || n64 > cap || base < 0 || base + n64 > N) continue;   // the simulator reports the layout error
+        const int n = (int)n64;
+        if (tid == 0) kor_s = 0;
+        __syncthreads();
+        uint64_t* buf0 = seg_buf;
+        uint64_t* buf1 = seg_buf + cap;
+        uint32_t kor = 0;
+        for (int i = tid; i < n; i += SORT_THREADS) {
+            const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)bit[base + i] : 0u;
+            const uint32_t key = (uint32_t)priority_key(policy, s[base + i], o[base + i], a[base + i], b, O0, O1);
+            buf0[i] = ((uint64_t)key << 32) | (uint32_t)i;
+            kor |= key;
+        }
+        kor = __reduce_or_sync(0xffffffffu, kor);
+        if ((tid & 31) == 0 && kor) atomicOr(&kor_s, kor);
+        __syncthreads();
+        const uint32_t kall = kor_s;
+        const int bits = kall ? 32 - __clz(kall) : 0;
+        const int npass = (bits + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
+        const int ipt = (n + SORT_THREADS - 1) / SORT_THREADS;
+        for (int p = 0; p < npass; ++p) {
+            seg_pass<SORT_THREADS>(buf0, buf1, n, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
+            uint64_t* t = buf0; buf0 = buf1; buf1 = t;
+        }
+        for (int p = tid; p < n; p += SORT_THREADS) {
+            const uint32_t id = (uint32_t)buf0[p];
+            order[base + p] = id;
+            rank[base + id] = (uint32_t)p;
+            if (req) req[base + p] = make_int4(s[base + id], o[base + id], (int)id, a[base + id]);
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
 
 int sm_count()
@@ -341,6 +460,29 @@ int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int6
                                                               w.hist + p * SORT_RADIX);
         ++*launches;
     }
+    return (int)cudaGetLastError();
+}
+
+int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
+                  const int32_t* s, const int32_t* o, const int32_t* a, const uint8_t* bit, int32_t O0,
+                  int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st, int64_t* launches)
+{
+    if (I <= 0 || N <= 0) return 0;
+    if (max_instance > SEG_SORT_MAX) return (int)cudaErrorInvalidValue;
+    const int cap = (int)((max_instance > 0 ? max_instance : 1) + 1) / 2 * 2;
+    const size_t smem = (size_t)2 * cap * sizeof(uint64_t);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_seg_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * SEG_SORT_MAX * (int)sizeof(uint64_t));
+        attr_set = true;
+    }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort, SORT_THREADS, smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    int64_t grid = (int64_t)per_sm * sm_count();
+    if (grid > I) grid = I;
+    k_seg_sort<<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, a, bit, O0, O1, order, rank, req);
+    ++*launches;
     return (int)cudaGetLastError();
 }
 
