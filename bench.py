@@ -4,10 +4,11 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A STEP is one pass of the whole hot path (keys -> pack -> segmented onesweep sort -> admission /
-feasibility -> state advance -> reductions) over one synthetic batch:
-`svf_simulate` under all four policies (SVF, 1-bit SVF, SJF, FCFS) on BASELINE.json configs[2]
-(4,096 instances x 1,000 requests, Poisson rate 4, M = 300,000), every output requested.
+A STEP is one pass of the whole hot path (keys -> pack -> per-instance radix sort -> admission /
+feasibility -> state advance -> reductions) over one synthetic batch: one
+`svf_simulate_policies` call = the simulator under all four policies (SVF, 1-bit SVF, SJF, FCFS) on
+BASELINE.json configs[2] (4,096 instances x 1,000 requests, Poisson rate 4, M = 300,000), every
+output requested.
 metric = simulated request-steps per second, request_steps = sum_i o_i per policy run.
 Per rank the batch is fixed (weak scaling); ranks hold different seeded batches; no collective
 on the data path (instances are independent).
@@ -44,9 +45,9 @@ L2_FLUSH_BYTES = 512 << 20
 # kernel's counting variant on the same inputs.  Peak = the SM issue rate, from the guide's unit
 # counts: SMs x 4 schedulers x 32 lanes x 1 warp-instruction/cycle x max SM clock.
 OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
-# HBM bytes per request the same kernel must move: a, s, o (12) + rank (4) + (s, o, id, a) record
-# in priority order (16) + start, finish (8) + latency word for p99 (8)
-SIM_BYTES_PER_REQUEST = 48
+# HBM bytes per request and policy the same kernel must move: a, s, o (12) + rank (4) + order (4) +
+# start, finish (8) + latency for the p99 selection (4 written, 4 read back)
+SIM_BYTES_PER_REQUEST = 36
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/r01_kslots_full.md
 SIM_DRAM_TRAFFIC_BYTES = 175.7e6
@@ -221,18 +222,16 @@ def run_ours(args):
     rs_step = batch.request_steps * len(POLICIES)
     dt_dev = B.DeviceTrace.from_host(batch, device=dev)
     outs = [B.SimOut.alloc(dt_dev) for _ in POLICIES]
-    ws = torch.empty(B.svf_simulate_workspace_bytes(dt_dev), dtype=torch.uint8, device=dev)
+    ws = torch.empty(B.svf_simulate_policies_workspace_bytes(dt_dev, len(POLICIES)), dtype=torch.uint8, device=dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
 
     def step(profile=None):
-        launches = 0
-        for i, p in enumerate(POLICIES):
-            B.svf_simulate(dt_dev, p, out=outs[i], ws=ws)
-            launches += B.last_launch_count(2)
-            if profile is not None:
-                profile.append(B.simulate_phase_ms())
-        return launches
+        # one call: presort under each policy, then ONE persistent launch over 4 x I work items
+        B.svf_simulate_policies(dt_dev, POLICIES, outs=outs, ws=ws)
+        if profile is not None:
+            profile.append(B.simulate_phase_ms())
+        return B.last_launch_count(2)
 
     def barrier():
         if world > 1:
@@ -273,7 +272,7 @@ def run_ours(args):
         step(profile=phase)
     B.set_profiling(False)
     phase = np.array(phase, dtype=np.float64)            # [calls, 4]
-    sim_ms = float(phase[:, 1].mean())                   # one k_sim launch, averaged over policies
+    sim_ms = float(phase[:, 1].mean())                   # the one k_sim_slots launch of a step (all four policies)
     share = {"phase_a_keys_sort_rank": float(phase[:, 0].sum() / phase[:, 3].sum()),
              "phase_b_simulator": float(phase[:, 1].sum() / phase[:, 3].sum()),
              "phase_c_p99": float(phase[:, 2].sum() / phase[:, 3].sum())}
@@ -287,8 +286,8 @@ def run_ours(args):
 
     def e2e_step():
         d = B.DeviceTrace.from_host(batch, device=dev, pinned=pinned, non_blocking=True)
-        for i, p in enumerate(POLICIES):
-            B.svf_simulate(d, p, out=outs[i], ws=ws)
+        B.svf_simulate_policies(d, POLICIES, outs=outs, ws=ws)
+        for i in range(len(POLICIES)):
             for k in B.RESULT_FIELDS:
                 host_out[i][k].copy_(getattr(outs[i], k), non_blocking=True)
         torch.cuda.synchronize()
@@ -315,19 +314,16 @@ def run_ours(args):
 
     # ---- algorithmic work of the dominant kernel, counted by its counting variant (untimed) ----
     B.set_profiling(2)
-    E = U = 0
-    for i, p in enumerate(POLICIES):
-        B.svf_simulate(dt_dev, p, out=outs[i], ws=ws)
-        e_, u_ = B.simulate_work_counts()
-        E += e_; U += u_
+    B.svf_simulate_policies(dt_dev, POLICIES, outs=outs, ws=ws)
+    E, U = B.simulate_work_counts()
     B.set_profiling(False)
-    ops_per_launch = (OPS_PER_EXAMINED * E + OPS_PER_UPDATED * U) / len(POLICIES)
+    ops_per_launch = OPS_PER_EXAMINED * E + OPS_PER_UPDATED * U
 
     ms_per_step = total_ms / args.steps
     value = rs_all / (ms_per_step * 1e-3)
     hbm_peak, hbm_src = measured_peaks()
     peak_ops, peak_src = alu_peak(torch, dev)
-    sim_bytes = SIM_BYTES_PER_REQUEST * batch.n_requests
+    sim_bytes = SIM_BYTES_PER_REQUEST * batch.n_requests * len(POLICIES)
     achieved = ops_per_launch / (sim_ms * 1e-3)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -346,8 +342,8 @@ def run_ours(args):
                      "frac": achieved / peak_ops, "traffic": SIM_DRAM_TRAFFIC_BYTES,
                      "peak_source": peak_src,
                      "algorithmic_ops_per_launch": ops_per_launch,
-                     "entries_examined_per_launch": E / len(POLICIES),
-                     "entries_updated_per_launch": U / len(POLICIES),
+                     "entries_examined_per_launch": E,
+                     "entries_updated_per_launch": U,
                      "kernel_ms": sim_ms, "share_of_step": share,
                      "hbm": {"algorithmic_bytes_per_launch": sim_bytes,
                              "achieved_gbs": sim_bytes / (sim_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,

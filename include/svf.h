@@ -118,12 +118,24 @@ int svf_admit(int policy, int64_t M, int32_t t,
  * Per instance, from t = a_0:  COMPLETE (k_i + o_i == t) -> ARRIVE (a_i <= t) -> ADMIT (pop
  * the head of the (key, arrival, id) order while the forward-looking check passes; stop at the
  * first blocked head) -> t+1  (event order: R1), until every request has finished.
- * Device-wide phase: validate + keys + one segmented onesweep radix sort giving every
- * instance its priority order; then one persistent kernel, one thread group per instance.
+ * Presort: keys + a stable radix sort giving every instance its priority order (in shared
+ * memory, one CTA per instance, when no instance has more than 4096 requests; else one
+ * device-wide segmented onesweep sort); then one persistent kernel, one thread group per
+ * instance, which also validates the data and selects p99.
  * `trace` and `out` are HOST structs holding DEVICE pointers (see above). */
 size_t svf_simulate_workspace_bytes(const svf_trace_t* trace);
 int svf_simulate(const svf_trace_t* trace, int policy, int64_t M, const svf_result_t* out,
                  void* ws, size_t ws_bytes, void* stream);
+
+/* The same simulator under SEVERAL policies in one call (the paper compares SVF, 1-bit SVF, SJF
+ * and FCFS on the same workload): policies[0 .. n_policies) [host], 1 <= n_policies <= 8,
+ * results of policies[k] in outs[k] ([host] array of structs holding DEVICE pointers; output
+ * buffers of different policies must not overlap).  Same semantics and error behaviour as
+ * n_policies calls of svf_simulate; the instances of all policies share ONE persistent launch
+ * (n_policies x I work items), which keeps the GPU full when I alone is only a wave or two. */
+size_t svf_simulate_policies_workspace_bytes(const svf_trace_t* trace, int n_policies);
+int svf_simulate_policies(const svf_trace_t* trace, int n_policies, const int* policies, int64_t M,
+                          const svf_result_t* outs, void* ws, size_t ws_bytes, void* stream);
 
 /* The sort subsystem on its own (a3), for tests and measurement: ascending, stable LSD
  * onesweep radix sort of n 64-bit words on the bit range [bit_lo, bit_hi) (0 <= bit_lo <
@@ -140,9 +152,10 @@ int64_t svf_last_launch_count(int which);
 
 /* Measurement aids.  svf_set_profiling(1): later svf_simulate calls on this host thread record
  * CUDA events on their stream around the three phases.  svf_simulate_phase_ms waits for the
- * events of the last such call and writes ms_out ([host] float[4]): [0] phase A (keys + pack +
- * segmented sort + rank), [1] phase B (the persistent simulator kernel), [2] phase C (p99 sort +
- * gather; 0 if not requested), [3] the whole call.  Returns SVF_EINVAL if profiling was off.
+ * events of the last such call and writes ms_out ([host] float[4]): [0] phase A (keys +
+ * presort + rank, every policy of the call), [1] phase B (the persistent simulator kernel), [2]
+ * phase C (p99 sort + gather of the M >= 2^30 kernel; else 0: p99 is selected inside the simulator
+ * kernel), [3] the whole call.  Returns SVF_EINVAL if profiling was off.
  * svf_set_profiling(2): as 1, and the simulator kernel also counts its algorithmic work (a
  * slower variant of the same kernel, same results; M < 2^30 only): svf_simulate_work_counts
  * synchronises and writes counts_out ([host] uint64[2]): [0] E = running entries examined,

@@ -22,7 +22,8 @@ OK, EINVAL, EWORKSPACE, ECUDA = 0, 1, 2, 3
 ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
 EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_workspace_bytes",
-           "svf_simulate", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
+           "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies",
+           "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
            "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
            "svf_simulate_work_counts")
 
@@ -71,6 +72,11 @@ def lib():
         L.svf_simulate.restype = C.c_int
         L.svf_simulate.argtypes = [C.POINTER(_Trace), C.c_int, C.c_int64, C.POINTER(_Result),
                                    C.c_void_p, C.c_size_t, C.c_void_p]
+        L.svf_simulate_policies_workspace_bytes.restype = C.c_size_t
+        L.svf_simulate_policies_workspace_bytes.argtypes = [C.POINTER(_Trace), C.c_int]
+        L.svf_simulate_policies.restype = C.c_int
+        L.svf_simulate_policies.argtypes = [C.POINTER(_Trace), C.c_int, C.POINTER(C.c_int), C.c_int64,
+                                            C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
         L.svf_sort_workspace_bytes.restype = C.c_size_t
         L.svf_sort_workspace_bytes.argtypes = [C.c_int64, C.c_int, C.c_int]
         L.svf_sort_words.restype = C.c_int
@@ -323,3 +329,32 @@ def svf_simulate(dt: DeviceTrace, policy: int, M: Optional[int] = None, out: Opt
     _check(rc, "svf_simulate")
     out._ws = ws  # keep the scratch alive until the caller drops the result
     return out
+
+
+def svf_simulate_policies_workspace_bytes(dt: DeviceTrace, n_policies: int) -> int:
+    tr = dt.c_struct()
+    return int(lib().svf_simulate_policies_workspace_bytes(C.byref(tr), int(n_policies)))
+
+
+def svf_simulate_policies(dt: DeviceTrace, policies, M: Optional[int] = None, outs=None,
+                          ws: Optional[torch.Tensor] = None, want=RESULT_FIELDS, stream=None):
+    """Enqueue the batched simulation under several policies in one call (one persistent launch
+    over len(policies) x I work items); returns the list of SimOut, one per policy."""
+    if not dt.offsets.is_cuda:
+        raise TypeError("svf_simulate_policies needs device tensors (the library has no CPU path)")
+    policies = [int(p) for p in policies]
+    M = dt.M if M is None else int(M)
+    if outs is None:
+        outs = [SimOut.alloc(dt, want) for _ in policies]
+    need = svf_simulate_policies_workspace_bytes(dt, len(policies))
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 256), dtype=torch.uint8, device=dt.offsets.device)
+    tr = dt.c_struct()
+    res = (_Result * len(policies))(*[o.c_struct() for o in outs])
+    pol = (C.c_int * len(policies))(*policies)
+    rc = lib().svf_simulate_policies(C.byref(tr), len(policies), pol, M, res, C.c_void_p(ws.data_ptr()),
+                                     ws.numel(), _stream(stream))
+    _check(rc, "svf_simulate_policies")
+    for o in outs:
+        o._ws = ws
+    return outs

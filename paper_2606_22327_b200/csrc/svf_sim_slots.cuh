@@ -113,20 +113,30 @@ __device__ __forceinline__ int qreg_first_ge(uint32_t word, int q)
     return l * 32 + (__ffs(wv) - 1);
 }
 
-struct SlotArgs {
-    int64_t I, N, M, max_instance;
-    int policy; int32_t O0, O1;
-    const int64_t* off;
-    const int32_t *a, *s, *o;
-    const uint8_t* bit;
-    const int4* req;                 // [N] (s, o, id, a) at (instance offset + rank)
+// per-policy inputs (the presorted order) and outputs of one launch
+struct PolicyIO {
+    int policy;
+    const int4* req;                 // [N] (s, o, id, a) at (instance offset + rank); NULL under QREG
     const uint32_t* rank;            // [N] rank of (instance offset + local id)
     const uint32_t* order;           // [N] local id at (instance offset + rank)
     int32_t *start, *finish;
     int64_t *tel, *peak, *rounds, *decisions;
+    int64_t* p99;                    // [I] or NULL
     int32_t *makespan, *status;
     uint32_t* lat;                   // [N] latency of (instance offset + local id): scratch of the p99 selection
-    int64_t* p99;                    // [I] or NULL
+};
+constexpr int MAX_POLICIES = 8;
+
+// One launch simulates n_policies x I work items (policy-major): a batch is usually compared
+// under several policies, and one long queue of items keeps the tail of the launch short.
+struct SlotArgs {
+    int64_t I, N, M, max_instance;
+    int32_t O0, O1;
+    const int64_t* off;
+    const int32_t *a, *s, *o;
+    const uint8_t* bit;
+    int n_policies;
+    PolicyIO io[MAX_POLICIES];
     unsigned long long* work_ctr;
     unsigned long long* work_counts; // [2] E, U (only written by the COUNT variant)
     char* gstate; size_t slot_bytes; // per-CTA state when it does not fit in shared memory
@@ -266,15 +276,20 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
     uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QREG_RANKS * 8);  // QREG only
     const int Mi = (int)g.M;
-    const bool want_start = g.start != nullptr, want_finish = g.finish != nullptr, want_p99 = g.p99 != nullptr;
+    const int64_t n_items = g.I * g.n_policies;
 
     while (true) {
         if (tid == 0) inst_s = (long long)atomicAdd(g.work_ctr, 1ull);
         __syncthreads();
-        const int64_t j = inst_s;
+        const int64_t item = inst_s;
         __syncthreads();
-        if (j >= g.I) break;
+        if (item >= n_items) break;
+        const int pi = (int)(item / g.I);            // policy-major
+        const int64_t j = item - (int64_t)pi * g.I;
 
+        const PolicyIO& io = g.io[pi];
+        const int policy = io.policy;
+        const bool want_start = io.start != nullptr, want_finish = io.finish != nullptr, want_p99 = io.p99 != nullptr;
         const int64_t base = g.off[j];
         const int64_t n64 = g.off[j + 1] - base;
         uint32_t flags = 0;
@@ -294,8 +309,8 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             if (oi < 1 || si < 0 || ai < 0) flags |= F_RANGE;
             if (i > 0 && ai < a[i - 1]) flags |= F_UNSORTED;
             if ((int64_t)si + oi > g.M) flags |= F_INFEASIBLE;
-            const uint32_t b = g.policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
-            if (oi >= 1 && si >= 0 && ai >= 0 && (priority_key(g.policy, si, oi, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
+            const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
+            if (oi >= 1 && si >= 0 && ai >= 0 && (priority_key(policy, si, oi, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
             max_a = ai > max_a ? ai : max_a;
         }
@@ -313,16 +328,16 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
 
         if (status != SVF_OK || n == 0) {
             for (int i = tid; i < n; i += THREADS) {
-                if (want_start) g.start[base + i] = -1;
-                if (want_finish) g.finish[base + i] = -1;
+                if (want_start) io.start[base + i] = -1;
+                if (want_finish) io.finish[base + i] = -1;
             }
         } else {
-            const uint32_t* __restrict__ rnk = g.rank + base;
-            const uint32_t* __restrict__ ord = g.order + base;
-            const int4* __restrict__ req = g.req + base;
-            int32_t* __restrict__ out_start = g.start + base;
-            int32_t* __restrict__ out_finish = g.finish + base;
-            uint32_t* out_lat = g.lat + base;
+            const uint32_t* __restrict__ rnk = io.rank + base;
+            const uint32_t* __restrict__ ord = io.order + base;
+            const int4* __restrict__ req = io.req + base;
+            int32_t* __restrict__ out_start = io.start + base;
+            int32_t* __restrict__ out_finish = io.finish + base;
+            uint32_t* out_lat = io.lat + base;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
             uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32)
             if (QREG) {
@@ -596,13 +611,13 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             mk = __reduce_max_sync(FULL, mk);
         }
         if (tid == 0) {
-            if (g.tel) g.tel[j] = tel;
-            if (g.peak) g.peak[j] = (int64_t)peak;
-            if (g.p99) g.p99[j] = p99v;
-            if (g.rounds) g.rounds[j] = (int64_t)rounds;
-            if (g.decisions) g.decisions[j] = (int64_t)decisions;
-            if (g.makespan) g.makespan[j] = mk;
-            if (g.status) g.status[j] = status;
+            if (io.tel) io.tel[j] = tel;
+            if (io.peak) io.peak[j] = (int64_t)peak;
+            if (io.p99) io.p99[j] = p99v;
+            if (io.rounds) io.rounds[j] = (int64_t)rounds;
+            if (io.decisions) io.decisions[j] = (int64_t)decisions;
+            if (io.makespan) io.makespan[j] = mk;
+            if (io.status) io.status[j] = status;
         }
         G::sync();
     }

@@ -279,13 +279,14 @@ __global__ void k_sim_p99(int64_t I, const int64_t* __restrict__ off, const Sort
 
 struct SimWs {
     SortWs sort;            // sized for the larger of the two sorts
-    uint64_t* words0;       // [N]
+    uint64_t* words0;       // [N] sort ping-pong (device-wide presort, p99 sort of the wide kernel)
     uint64_t* words1;       // [N]
-    uint32_t* order;        // [N]
-    uint32_t* rank;         // [N]
-    int4* req;              // [N]
+    uint32_t* order[MAX_POLICIES];    // [N] each
+    uint32_t* rank[MAX_POLICIES];     // [N] each
+    int4* req[MAX_POLICIES];          // [N] each
+    uint32_t* lat[MAX_POLICIES];      // [N] each: latencies for the in-kernel p99 selection
+    int32_t* status_tmp[MAX_POLICIES];// [I] each, when the caller does not want status
     unsigned long long* counts;   // [2] E, U of the counting variant
-    int32_t* status_tmp;    // [I] when the caller does not want status
     unsigned long long* work_ctr;
     char* gstate;
     size_t slot_bytes;
@@ -312,7 +313,7 @@ constexpr size_t SMEM_STATE_LIMIT = 200 * 1024;
 constexpr size_t SMEM_WARP_STATE_LIMIT = 12 * 1024;   // one-warp groups: keep >= 16 CTAs per SM
 constexpr int SLOT_K = 16;                            // register slots per thread
 
-SimConfig sim_config(const svf_trace_t* tr, int64_t M)
+SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
 {
     SimConfig c;
     const int64_t I = tr->n_instances, mx = tr->max_instance > 0 ? tr->max_instance : 1;
@@ -326,7 +327,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M)
     // group width: enough warps in flight to cover the GPU (about 16 per SM), no wider than the
     // running set can use
     const int64_t target_warps = (int64_t)sm_count() * 16;
-    int64_t w = I > 0 ? target_warps / I : 1;
+    int64_t w = I > 0 ? target_warps / (I * (P > 0 ? P : 1)) : 1;   // P policies share one launch
     int threads = 32;
     const int tmax = c.slots ? 256 : 1024;
     while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
@@ -423,8 +424,8 @@ int sim_grid_any(const SimConfig& c, int64_t I)
     }
 }
 
-// workspace layout; `grid` < 0: size for the worst case without touching the device
-void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig& c, int grid_slots)
+// workspace layout for P policies; base may be nullptr (sizes only)
+void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig& c, int grid_slots, int P)
 {
     const int64_t N = tr->n_requests, I = tr->n_instances;
     size_t p = 0;
@@ -437,11 +438,14 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
     p += align_up(sort_bytes, 256);
     w->words0 = (uint64_t*)(base + p); p += align_up((size_t)N * 8, 256);
     w->words1 = (uint64_t*)(base + p); p += align_up((size_t)N * 8, 256);
-    w->order = (uint32_t*)(base + p);  p += align_up((size_t)N * 4, 256);
-    w->rank = (uint32_t*)(base + p);   p += align_up((size_t)N * 4, 256);
-    w->req = (int4*)(base + p);        p += align_up((size_t)N * 16, 256);
+    for (int q = 0; q < P; ++q) {
+        w->order[q] = (uint32_t*)(base + p);  p += align_up((size_t)N * 4, 256);
+        w->rank[q] = (uint32_t*)(base + p);   p += align_up((size_t)N * 4, 256);
+        w->req[q] = (int4*)(base + p);        p += align_up((size_t)N * 16, 256);
+        w->lat[q] = (uint32_t*)(base + p);    p += align_up((size_t)N * 4, 256);
+        w->status_tmp[q] = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
+    }
     w->counts = (unsigned long long*)(base + p); p += 256;
-    w->status_tmp = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
     w->work_ctr = (unsigned long long*)(base + p); p += 256;
     w->slot_bytes = c.gslot_bytes;
     w->grid_slots = grid_slots;
@@ -472,120 +476,52 @@ int64_t sim_last_launches() { return g_launches_sim; }
 
 using namespace svf;
 
-extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr)
+namespace svf {
+namespace {
+
+size_t sim_workspace_bytes(const svf_trace_t* tr, int P)
 {
-    if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0) return 0;
-    // M is not known here: size for the larger of the two kernels' layouts.  State slots in
-    // global memory only exist for oversized instances, at most 2 CTAs per SM.
+    if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0 || P < 1 || P > MAX_POLICIES) return 0;
+    // M is not known here: size for the larger of the two kernels' layouts
     size_t need = 0;
     for (int64_t M : {(int64_t)0, (int64_t)1 << 30}) {
-        SimConfig c = sim_config(tr, M);
+        SimConfig c = sim_config(tr, M, P);
         SimWs w;
         int64_t slots = c.gslot_bytes ? (int64_t)c.max_cta_per_sm * sm_count() : 0;
-        if (slots > tr->n_instances) slots = tr->n_instances;
-        sim_ws_layout(&w, nullptr, tr, c, (int)slots);
+        if (slots > tr->n_instances * P) slots = tr->n_instances * P;
+        sim_ws_layout(&w, nullptr, tr, c, (int)slots, P);
         need = w.total > need ? w.total : need;
     }
     return need + 256;
 }
 
-extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out,
-                            void* ws, size_t ws_bytes, void* stream)
+// the wide sorted-array kernel (M >= 2^30): one policy per call
+int simulate_wide(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out, const SimConfig& c,
+                  SimWs& w, int grid, cudaStream_t st)
 {
-    g_launches_sim = 0;
-    if (!tr || !out) return SVF_EINVAL;
     const int64_t I = tr->n_instances, N = tr->n_requests;
-    if (I < 0 || N < 0 || N >= ((int64_t)1 << 30) || tr->max_instance < 0 || tr->max_instance > N) return SVF_EINVAL;
-    if (policy < 0 || policy > 3 || M < 0) return SVF_EINVAL;
-    if (policy == SVF_SVF_1BIT && ((N > 0 && !tr->bit) || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
-    if (I == 0) return SVF_OK;
-    if (!tr->offsets || (N > 0 && (!tr->arrival || !tr->prompt || !tr->output))) return SVF_EINVAL;
-    SimConfig c = sim_config(tr, M);
-    if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;          // packed sort word would not fit (DESIGN.md 5)
-    if (!ws) return SVF_EWORKSPACE;
-    cudaStream_t st = (cudaStream_t)stream;
-
-    int dev_count = 0;
-    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
-
-    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
-    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
-    int grid = sim_grid_any(c, I);
-    if (c.gslot_bytes && grid > c.max_cta_per_sm * sm_count()) grid = c.max_cta_per_sm * sm_count();
-    SimWs w;
-    sim_ws_layout(&w, base, tr, c, c.gslot_bytes ? grid : 0);
-    if (w.total > avail) return SVF_EWORKSPACE;
-
     SimArgs g;
     g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
     g.policy = policy; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
     g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
-    g.order = w.order; g.rank = w.rank; g.req = (c.slots && c.qreg) ? nullptr : w.req;
+    g.order = w.order[0]; g.rank = w.rank[0]; g.req = w.req[0];
     g.start = out->start; g.finish = out->finish; g.tel = out->total_latency; g.peak = out->peak_kv;
     g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
-    g.status = out->status ? out->status : w.status_tmp;
+    g.status = out->status ? out->status : w.status_tmp[0];
     g.latw = out->p99_latency ? w.words0 : nullptr;
     g.work_ctr = w.work_ctr; g.gstate = w.gstate; g.slot_bytes = w.slot_bytes; g.cap = c.cap;
-
-    g_events_valid = false;
-    prof_mark(0, st);
     if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
-    int rc = 0;
-    if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
-        // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance
-        rc = seg_sort_keys(policy, I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->arrival,
-                           tr->bit, tr->O0, tr->O1, w.order, w.rank, g.req, st, &g_launches_sim);
-        if (rc) return SVF_ECUDA;
-    } else if (N > 0) {
+    if (N > 0) {
         int64_t blocks = ceil_div(N, 256);
         const int64_t capb = (int64_t)sm_count() * 8;
         if (blocks > capb) blocks = capb;
         k_sim_pack<<<(unsigned)blocks, 256, 0, st>>>(g, w.words0);
         ++g_launches_sim;
-        rc = sort_u64(w.sort, w.words0, w.words1, w.words0, N, c.sort_lo, c.sort_hi, st, &g_launches_sim);
-        if (rc) return SVF_ECUDA;
-        k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order, w.rank);
+        if (sort_u64(w.sort, w.words0, w.words1, w.words0, N, c.sort_lo, c.sort_hi, st, &g_launches_sim)) return SVF_ECUDA;
+        k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order[0], w.rank[0]);
         ++g_launches_sim;
     }
     prof_mark(1, st);
-    if (c.slots) {
-        SlotArgs q;
-        q.I = I; q.N = N; q.M = M; q.max_instance = tr->max_instance;
-        q.policy = policy; q.O0 = tr->O0; q.O1 = tr->O1;
-        q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
-        q.req = w.req; q.rank = w.rank; q.order = w.order;
-        q.start = g.start; q.finish = g.finish; q.tel = g.tel; q.peak = g.peak; q.rounds = g.rounds;
-        q.decisions = g.decisions; q.makespan = g.makespan; q.status = g.status;
-        q.lat = reinterpret_cast<uint32_t*>(w.words0); q.p99 = out->p99_latency;   // p99 selected in the kernel
-        q.work_ctr = w.work_ctr; q.work_counts = w.counts;
-        q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
-        const bool count = g_profiling == 2;
-        if (count) {
-            if (cudaMemsetAsync(w.counts, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
-            g_counts_dev = w.counts;
-        }
-#define SVF_SLOTS_LAUNCH(T, S, Q)                                                         \
-        do {                                                                                  \
-            if (count) k_sim_slots<T, SLOT_K, S, true, Q><<<grid, T, c.dyn_smem, st>>>(q);    \
-            else       k_sim_slots<T, SLOT_K, S, false, Q><<<grid, T, c.dyn_smem, st>>>(q);   \
-        } while (0)
-        if (c.qreg) {
-            SVF_SLOTS_LAUNCH(32, true, true);
-        } else if (c.smem) {
-            switch (c.threads) {
-            case 32: SVF_SLOTS_LAUNCH(32, true, false); break;
-            case 128: SVF_SLOTS_LAUNCH(128, true, false); break;
-            default: SVF_SLOTS_LAUNCH(256, true, false); break;
-            }
-        } else {
-            switch (c.threads) {
-            case 32: SVF_SLOTS_LAUNCH(32, false, false); break;
-            case 128: SVF_SLOTS_LAUNCH(128, false, false); break;
-            default: SVF_SLOTS_LAUNCH(256, false, false); break;
-            }
-        }
-#undef SVF_SLOTS_LAUNCH
-    } else {
 #define SVF_SIM_LAUNCH(T, S) k_sim<T, S><<<grid, T, c.dyn_smem, st>>>(g)
     if (c.smem) {
         switch (c.threads) {
@@ -603,24 +539,155 @@ extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const 
         }
     }
 #undef SVF_SIM_LAUNCH
-    }
     ++g_launches_sim;
     if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
     prof_mark(2, st);
-
-    if (out->p99_latency && !c.slots) {
-        if (N > 0) {
-            rc = sort_u64(w.sort, w.words0, w.words1, w.words0, N, 0, 32 + c.ib, st, &g_launches_sim);
-            if (rc) return SVF_ECUDA;
-        } else {
-            rc = sort_u64(w.sort, w.words0, w.words1, w.words0, 0, 0, 32, st, &g_launches_sim);
-            if (rc) return SVF_ECUDA;
-        }
+    if (out->p99_latency) {
+        if (sort_u64(w.sort, w.words0, w.words1, w.words0, N > 0 ? N : 0, 0, N > 0 ? 32 + c.ib : 32, st, &g_launches_sim)) return SVF_ECUDA;
         k_sim_p99<<<(unsigned)ceil_div(I, 128), 128, 0, st>>>(I, tr->offsets, w.sort.plan, g.status, out->p99_latency);
         ++g_launches_sim;
     }
-    prof_mark(3, st);
     return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
+}
+
+int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, const svf_result_t* outs,
+                  void* ws, size_t ws_bytes, void* stream)
+{
+    if (!tr || !outs || !policies || P < 1 || P > MAX_POLICIES) return SVF_EINVAL;
+    const int64_t I = tr->n_instances, N = tr->n_requests;
+    if (I < 0 || N < 0 || N >= ((int64_t)1 << 30) || tr->max_instance < 0 || tr->max_instance > N) return SVF_EINVAL;
+    if (M < 0) return SVF_EINVAL;
+    for (int q = 0; q < P; ++q) {
+        if (policies[q] < 0 || policies[q] > 3) return SVF_EINVAL;
+        if (policies[q] == SVF_SVF_1BIT && ((N > 0 && !tr->bit) || tr->O0 < 1 || tr->O1 < 1)) return SVF_EINVAL;
+    }
+    if (I == 0) return SVF_OK;
+    if (!tr->offsets || (N > 0 && (!tr->arrival || !tr->prompt || !tr->output))) return SVF_EINVAL;
+    SimConfig c = sim_config(tr, M, P);
+    if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;          // packed sort word would not fit (DESIGN.md 5)
+    if (!ws) return SVF_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
+
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
+    int grid = sim_grid_any(c, I * P);
+    if (c.gslot_bytes && grid > c.max_cta_per_sm * sm_count()) grid = c.max_cta_per_sm * sm_count();
+    SimWs w;
+    sim_ws_layout(&w, base, tr, c, c.gslot_bytes ? grid : 0, P);
+    if (w.total > avail) return SVF_EWORKSPACE;
+
+    g_events_valid = false;
+    prof_mark(0, st);
+    if (!c.slots) {
+        // M >= 2^30: the wide kernel, one policy after the other
+        int rc = SVF_OK;
+        for (int q = 0; q < P && rc == SVF_OK; ++q) rc = simulate_wide(tr, policies[q], M, &outs[q], c, w, grid, st);
+        prof_mark(3, st);
+        return rc;
+    }
+
+    // ---- phase A: the priority order of every instance under every policy ---------------------
+    SlotArgs q;
+    q.I = I; q.N = N; q.M = M; q.max_instance = tr->max_instance;
+    q.O0 = tr->O0; q.O1 = tr->O1;
+    q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
+    q.n_policies = P;
+    if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
+    for (int k = 0; k < P; ++k) {
+        const svf_result_t* out = &outs[k];
+        PolicyIO& io = q.io[k];
+        io.policy = policies[k];
+        io.req = c.qreg ? nullptr : w.req[k];
+        io.rank = w.rank[k]; io.order = w.order[k];
+        io.start = out->start; io.finish = out->finish; io.tel = out->total_latency; io.peak = out->peak_kv;
+        io.rounds = out->rounds; io.decisions = out->decisions; io.p99 = out->p99_latency;
+        io.makespan = out->makespan; io.status = out->status;
+        io.lat = w.lat[k];
+        if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
+            // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance
+            if (seg_sort_keys(policies[k], I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->arrival,
+                              tr->bit, tr->O0, tr->O1, w.order[k], w.rank[k], c.qreg ? nullptr : w.req[k], st,
+                              &g_launches_sim))
+                return SVF_ECUDA;
+        } else if (N > 0) {
+            SimArgs g;
+            g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
+            g.policy = policies[k]; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
+            g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
+            g.req = c.qreg ? nullptr : w.req[k];
+            int64_t blocks = ceil_div(N, 256);
+            const int64_t capb = (int64_t)sm_count() * 8;
+            if (blocks > capb) blocks = capb;
+            k_sim_pack<<<(unsigned)blocks, 256, 0, st>>>(g, w.words0);
+            ++g_launches_sim;
+            if (sort_u64(w.sort, w.words0, w.words1, w.words0, N, c.sort_lo, c.sort_hi, st, &g_launches_sim)) return SVF_ECUDA;
+            k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order[k], w.rank[k]);
+            ++g_launches_sim;
+        }
+    }
+    prof_mark(1, st);
+
+    // ---- phase B: one persistent launch over P x I work items -------------------------------------
+    q.work_ctr = w.work_ctr; q.work_counts = w.counts;
+    q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
+    const bool count = g_profiling == 2;
+    if (count) {
+        if (cudaMemsetAsync(w.counts, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
+        g_counts_dev = w.counts;
+    }
+#define SVF_SLOTS_LAUNCH(T, S, Q)                                                         \
+    do {                                                                                  \
+        if (count) k_sim_slots<T, SLOT_K, S, true, Q><<<grid, T, c.dyn_smem, st>>>(q);    \
+        else       k_sim_slots<T, SLOT_K, S, false, Q><<<grid, T, c.dyn_smem, st>>>(q);   \
+    } while (0)
+    if (c.qreg) {
+        SVF_SLOTS_LAUNCH(32, true, true);
+    } else if (c.smem) {
+        switch (c.threads) {
+        case 32: SVF_SLOTS_LAUNCH(32, true, false); break;
+        case 128: SVF_SLOTS_LAUNCH(128, true, false); break;
+        default: SVF_SLOTS_LAUNCH(256, true, false); break;
+        }
+    } else {
+        switch (c.threads) {
+        case 32: SVF_SLOTS_LAUNCH(32, false, false); break;
+        case 128: SVF_SLOTS_LAUNCH(128, false, false); break;
+        default: SVF_SLOTS_LAUNCH(256, false, false); break;
+        }
+    }
+#undef SVF_SLOTS_LAUNCH
+    ++g_launches_sim;
+    if (cudaGetLastError() != cudaSuccess) return SVF_ECUDA;
+    prof_mark(2, st);
+    prof_mark(3, st);       // phase C (p99) happens inside the kernel
+    return SVF_OK;
+}
+
+}  // namespace
+}  // namespace svf
+
+extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr) { return sim_workspace_bytes(tr, 1); }
+
+extern "C" size_t svf_simulate_policies_workspace_bytes(const svf_trace_t* tr, int n_policies)
+{
+    return sim_workspace_bytes(tr, n_policies);
+}
+
+extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out,
+                            void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches_sim = 0;
+    return simulate_impl(tr, 1, &policy, M, out, ws, ws_bytes, stream);
+}
+
+extern "C" int svf_simulate_policies(const svf_trace_t* tr, int n_policies, const int* policies, int64_t M,
+                                     const svf_result_t* outs, void* ws, size_t ws_bytes, void* stream)
+{
+    g_launches_sim = 0;
+    return simulate_impl(tr, n_policies, policies, M, outs, ws, ws_bytes, stream);
 }
 
 extern "C" void svf_set_profiling(int mode) { g_profiling = mode == 2 ? 2 : (mode ? 1 : 0); if (mode != 2) g_counts_dev = nullptr; }

@@ -82,6 +82,24 @@ def test_simulate_rejects_bad_host_arguments(svf_lib):
     L.svf_simulate_workspace_bytes.restype = C.c_size_t
     L.svf_simulate_workspace_bytes.argtypes = [C.POINTER(_Trace)]
     assert L.svf_simulate_workspace_bytes(C.byref(tr)) > 0
+    # several policies in one call
+    L.svf_simulate_policies.restype = C.c_int
+    L.svf_simulate_policies.argtypes = [C.POINTER(_Trace), C.c_int, C.POINTER(C.c_int), C.c_int64,
+                                        C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+    L.svf_simulate_policies_workspace_bytes.restype = C.c_size_t
+    L.svf_simulate_policies_workspace_bytes.argtypes = [C.POINTER(_Trace), C.c_int]
+    pol = (C.c_int * 2)(0, 3)
+    outs = (_Result * 2)()
+    assert L.svf_simulate_policies(C.byref(tr), 0, pol, 10, outs, None, 0, None) == 1     # n_policies < 1
+    assert L.svf_simulate_policies(C.byref(tr), 9, pol, 10, outs, None, 0, None) == 1     # n_policies > 8
+    assert L.svf_simulate_policies(C.byref(tr), 2, None, 10, outs, None, 0, None) == 1    # null policies
+    bad = (C.c_int * 2)(0, 7)
+    assert L.svf_simulate_policies(C.byref(tr), 2, bad, 10, outs, None, 0, None) == 1     # unknown policy
+    assert L.svf_simulate_policies(C.byref(tr), 2, pol, 10, outs, None, 0, None) == 1     # null offsets
+    w1 = L.svf_simulate_policies_workspace_bytes(C.byref(tr), 1)
+    w4 = L.svf_simulate_policies_workspace_bytes(C.byref(tr), 4)
+    assert w1 == L.svf_simulate_workspace_bytes(C.byref(tr)) and w4 > w1
+    assert L.svf_simulate_policies_workspace_bytes(C.byref(tr), 0) == 0
 
 
 def test_binding_refuses_cpu_tensors(svf_lib):

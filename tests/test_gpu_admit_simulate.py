@@ -202,6 +202,39 @@ def test_group_widths_and_state_placement(B, oracle):
             check(B, oracle, tr, policy, ctx=f"I={I} n={n}")
 
 
+def test_policies_in_one_call(B, oracle):
+    """svf_simulate_policies: one launch over n_policies x I work items == separate calls == oracle,
+    for each kernel family (warp + register bitmap, CTA + shared bitmap, wide kernel for M >= 2^30)."""
+    import torch
+    cases = [(T.config3(n_instances=300, n=200, lam=4.0, M=60_000), None, [0, 1, 2, 3]),
+             (T.config3(n_instances=6, n=1500, lam=8.0, M=60_000), None, [3, 0, 2]),
+             (T.config5(n_instances=3, n=5000, M=200_000, p_flip=0.2), None, [1, 0]),
+             (T.config3(n_instances=20, n=100, lam=4.0), 1 << 30, [0, 3])]
+    for tr, M, pols in cases:
+        dt = B.DeviceTrace.from_host(tr)
+        outs = B.svf_simulate_policies(dt, pols, M)
+        torch.cuda.synchronize()
+        for pol, out in zip(pols, outs):
+            ref = oracle.simulate(tr, pol, M=M, n_threads=8)
+            got = {k: getattr(out, k).cpu().numpy() for k in FIELDS}
+            assert_same(got, ref, tr, f"{tr.name} policies={pols} policy {pol}")
+
+
+def test_policies_call_with_rejected_and_empty_instances(B, oracle):
+    import torch
+    parts = [T.random_small(7, 12, 9, 11, 24, a_hi=10), T.random_small(8, 0, 9, 11, 24),
+             T.random_small(9, 30, 9, 11, 24, a_hi=3)]
+    parts[2].output[4] = 0                              # ERANGE in instance 2
+    tr = T.concat(parts, "mixed", 24, 3, 9)
+    dt = B.DeviceTrace.from_host(tr)
+    outs = B.svf_simulate_policies(dt, [2, 1])
+    torch.cuda.synchronize()
+    for pol, out in zip([2, 1], outs):
+        ref = oracle.simulate(tr, pol)
+        assert_same({k: getattr(out, k).cpu().numpy() for k in FIELDS}, ref, tr, f"mixed policy {pol}")
+    assert int(outs[0].status[2]) != 0
+
+
 def test_outputs_are_optional(B, oracle):
     tr = T.config3(n_instances=8, lam=4.0)
     ref = oracle.simulate(tr, 0)
