@@ -429,19 +429,16 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 }
                 if (arrived) {
                     if (QREG) {
-                        // reload the bitmap word and take head and second from it
+                        // reload the bitmap word; the head is its lowest set bit (arrivals set bits)
                         __syncwarp();
                         qword = qbits[lane];
-                        const int r0 = qreg_first_ge(qword, 0);
+                        const uint32_t nz = __ballot_sync(FULL, qword != 0u);
+                        const int l0 = __ffs(nz) - 1;
+                        const int r0 = l0 * 32 + (__ffs(__shfl_sync(FULL, qword, l0)) - 1);
                         if (r0 != head.r) {
                             const int2 v = qrec[r0];
                             head.r = r0; head.s = v.x; head.o = v.y;
                             t_lb = t;                     // a new head: evaluate it now
-                        }
-                        const int r1 = qreg_first_ge(qword, r0 + 1);
-                        if (r1 != second.r) {
-                            second.r = r1;
-                            if (r1 != INT_MAX) { const int2 v = qrec[r1]; second.s = v.x; second.o = v.y; }
                         }
                     } else if (THREADS == 32) {
                         __syncwarp();
@@ -452,10 +449,11 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                 if (head.r != INT_MAX) {
                     rounds += 1;
                     while (t >= t_lb) {
-                        // ---- evaluation pass -----------------------------------------------------
+                        // ---- evaluation pass (with the update applied speculatively) -------------
                         const int fh = t + head.o;
                         const uint32_t t1 = (uint32_t)t + 1u, oh = (uint32_t)head.o, fhu = (uint32_t)fh;
                         const uint32_t Kc = (uint32_t)head.s - (uint32_t)t - (uint32_t)Mi;   // s_h - t - M (mod 2^32)
+                        const uint32_t add = (uint32_t)head.s - (uint32_t)t;                  // A_j += s_h - t + f_j
                         uint32_t acc = 0, dm = 0;
                         int viol = INT_MIN;
                         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
@@ -464,36 +462,51 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
 #define SVF_EVAL(k) {                                                                          \
                             const uint32_t x = (uint32_t)f[k] - t1;                            \
                             if (f[k] >= fh) acc += c[k] + fhu;                                 \
-                            if (x < oh) viol = __viaddmax_s32((int)B[k], (int)Kc, viol);       \
+                            if (x < oh) {                                                      \
+                                viol = __viaddmax_s32((int)B[k], (int)Kc, viol);               \
+                                B[k] += add + (uint32_t)f[k];                                  \
+                                if (COUNT) cntU += 1;                                          \
+                            }                                                                  \
                             dm = __funnelshift_l(x, dm, 1);                                    \
                             if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
                         }
                         SVF_SLOT_GROUPS(g4, SVF_EVAL)
 #undef SVF_EVAL
-                        // lowest free register slot of this thread: bit k of dm = slot k is dead
-                        const int kfree = dm ? __ffs(dm) - 1 : 4 * g4;
-                        int fidx = kfree < K ? (kfree << TSHIFT) + tid : INT_MAX;
+                        // lowest free register slot of this thread as a one-hot bit (bit k of dm =
+                        // slot k is dead); the group takes the lowest (slot, thread) pair
+                        const uint32_t low = dm ? (dm & (0u - dm)) : (1u << (4 * g4));
+                        int fkey = low < (1u << K) ? (int)((low << TSHIFT) | (uint32_t)tid) : INT_MAX;
+                        int eidx = INT_MAX;
                         if (use_ext) {
                             for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                 const int e = q - REGCAP;
                                 const int fk = ef[e];
                                 const uint32_t x = (uint32_t)fk - t1;
                                 if (fk >= fh) acc += ec[e] + fhu;
-                                if (x < oh) viol = __viaddmax_s32((int)eB[e], (int)Kc, viol);
-                                if (x >> 31) fidx = fidx < q ? fidx : q;
+                                if (x < oh) {
+                                    viol = __viaddmax_s32((int)eB[e], (int)Kc, viol);
+                                    eB[e] += add + (uint32_t)fk;
+                                    if (COUNT) cntU += 1;
+                                }
+                                if (x >> 31) eidx = eidx < q ? eidx : q;
                                 if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
                             }
                         }
-                        reduce_add_max_min<THREADS>(acc, viol, fidx, red, rparity);
+                        reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
                         const int Ah = head.s + head.o + (int)acc;        // exact: 0 <= A_h <= 2M < 2^31
                         if (viol > 0 || Ah > Mi) {
-                            // ---- blocked (no bypass): how long at least? ------------------
+                            // ---- blocked (no bypass): take the update back and find how
+                            // long the head stays blocked at least --------------------------------
                             int wmax = 0, minge = INT_MAX;
 #define SVF_BLOCK(k) {                                                                         \
                                 const uint32_t x = (uint32_t)f[k] - t1;                        \
-                                const int v = (int)(B[k] + Kc), d = (int)x + 1;                \
-                                const int w = v < d ? v : d;                                   \
-                                if (x < oh) wmax = w > wmax ? w : wmax;                        \
+                                if (x < oh) {                                                  \
+                                    B[k] -= add + (uint32_t)f[k];                              \
+                                    const int v = (int)(B[k] + Kc), d = (int)x + 1;            \
+                                    const int w = v < d ? v : d;                               \
+                                    wmax = w > wmax ? w : wmax;                                \
+                                    if (COUNT) cntU -= 1;                                      \
+                                }                                                              \
                                 if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
                             }
                             SVF_SLOT_GROUPS(g4, SVF_BLOCK)
@@ -503,9 +516,13 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                                     const int e = q - REGCAP;
                                     const int fk = ef[e];
                                     const uint32_t x = (uint32_t)fk - t1;
-                                    const int v = (int)(eB[e] + Kc), d = (int)x + 1;
-                                    const int w = v < d ? v : d;
-                                    if (x < oh) wmax = w > wmax ? w : wmax;
+                                    if (x < oh) {
+                                        eB[e] -= add + (uint32_t)fk;
+                                        const int v = (int)(eB[e] + Kc), d = (int)x + 1;
+                                        const int w = v < d ? v : d;
+                                        wmax = w > wmax ? w : wmax;
+                                        if (COUNT) cntU -= 1;
+                                    }
                                     if (fk >= fh) minge = fk < minge ? fk : minge;
                                 }
                             }
@@ -517,32 +534,27 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             break;
                         }
 
-                        // ---- admit the head: update pass, then write it into slot idx ------------
-                        const int idx = fidx == INT_MAX ? hw : fidx;
-                        const uint32_t add = (uint32_t)head.s - (uint32_t)t;
+                        // ---- admitted: the update is already in place; write the head into a slot --
                         const uint32_t Bh = (uint32_t)Ah + fhu;
-#define SVF_UPDATE(k) {                                                                        \
-                            const uint32_t x = (uint32_t)f[k] - t1;                            \
-                            if (x < oh) { B[k] += add + (uint32_t)f[k]; if (COUNT) cntU += 1; } \
-                        }
-                        SVF_SLOT_GROUPS(g4, SVF_UPDATE)
-#undef SVF_UPDATE
-                        if (use_ext) {
-                            for (int q = REGCAP + tid; q < hw; q += THREADS) {
-                                const int e = q - REGCAP;
-                                const int fk = ef[e];
-                                if ((uint32_t)fk - t1 < oh) { eB[e] += add + (uint32_t)fk; if (COUNT) cntU += 1; }
-                            }
-                        }
-                        if (idx < REGCAP) {
-                            const bool mine = (idx & (THREADS - 1)) == tid;
-                            const int ik = idx >> TSHIFT;
+                        int idx;
+                        if (fkey != INT_MAX) {
+                            const int ik = 31 - __clz(fkey >> TSHIFT);           // uniform
+                            const bool mine = (fkey & (THREADS - 1)) == tid;
+                            idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
 #define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
                             SVF_PUT16(ik, SVF_PUT)
 #undef SVF_PUT
-                        } else if (((idx - REGCAP) & (THREADS - 1)) == tid) {
-                            const int e = idx - REGCAP;
-                            ef[e] = fh; eB[e] = Bh; ec[e] = add;
+                        } else {
+                            // every register slot is live: the lowest dead ext slot, else a new one
+                            if (use_ext) {
+                                uint32_t z = 0; int zmax = 0;
+                                reduce_add_max_min<THREADS>(z, zmax, eidx, red, rparity);
+                            }
+                            idx = eidx == INT_MAX ? hw : eidx;
+                            if (((idx - REGCAP) & (THREADS - 1)) == tid) {
+                                const int e = idx - REGCAP;
+                                ef[e] = fh; eB[e] = Bh; ec[e] = add;
+                            }
                         }
                         hw = idx + 1 > hw ? idx + 1 : hw;
                         {   // every final A_j is a mem(f_j): the new A_h and the raised in-range A_j
@@ -559,15 +571,19 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                         }
                         ++started; ++decisions;
                         if ((started & 31) == 0) flush(32);
-                        // promote the second; fetch the record behind it one admission ahead
-                        head = second;
-                        second.r = INT_MAX;
-                        if (head.r == INT_MAX) break;
                         if (QREG) {
-                            const int r = qreg_first_ge(qword, head.r + 1);
-                            second.r = r;
-                            if (r != INT_MAX) { const int2 v = qrec[r]; second.s = v.x; second.o = v.y; }
+                            // next head: the lowest set bit; its (s, o) come from shared memory
+                            const uint32_t nz = __ballot_sync(FULL, qword != 0u);
+                            if (!nz) { head.r = INT_MAX; break; }
+                            const int l0 = __ffs(nz) - 1;
+                            const int r = l0 * 32 + (__ffs(__shfl_sync(FULL, qword, l0)) - 1);
+                            const int2 v = qrec[r];
+                            head.r = r; head.s = v.x; head.o = v.y;
                         } else {
+                            // promote the second; fetch the record behind it one admission ahead
+                            head = second;
+                            second.r = INT_MAX;
+                            if (head.r == INT_MAX) break;
                             const int r = queue_first_ge(L0, L1, n, nL1, head.r + 1);
                             if (r != INT_MAX) {
                                 const int4 qv = req[r];
