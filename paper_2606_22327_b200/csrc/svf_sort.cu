@@ -11,11 +11,15 @@
 //    host never reads anything back (key bits are bounded: < 2^24..2^26 for the paper-shaped
 //    workloads).
 //  * Each pass CTA owns one 4096-word tile (32 KB): the tile is staged global->shared with one
-//    1-D TMA bulk copy (cp.async.bulk + mbarrier), ranked per warp with __match_any_sync digit
-//    ballots (stable), scattered inside shared memory so the final global stores are coalesced
-//    runs per digit.
-//  * Tile ids come from an atomic counter, so a tile's predecessors are always resident or
-//    done: the look-back spin cannot deadlock.
+//    1-D TMA bulk copy (cp.async.bulk + mbarrier); its digit counts are taken first (shared-memory
+//    atomics) and published as the tile's AGGREGATE before anything else, then the keys are ranked
+//    per warp with one ballot per digit bit (stable; no MATCH instruction: measured slower),
+//    scattered inside shared memory so the final global stores are coalesced runs per digit.
+//  * Decoupled look-back, eight predecessor words per round trip to L2 (independent loads consumed
+//    in order).  Tile ids come from an atomic counter, so a tile's predecessors are always
+//    resident or done: the look-back spin cannot deadlock.
+//  * The plan kernel ping-pongs the two buffers so that the last EXECUTED pass lands in the
+//    caller's output buffer: no copy afterwards.
 #include "svf_internal.cuh"
 
 namespace svf {
@@ -27,6 +31,28 @@ constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_INCL = 2u << 30, VALUE_MASK = (1u <
 __device__ __forceinline__ uint32_t digit_of(uint64_t w, int shift, uint32_t mask)
 {
     return (uint32_t)(w >> shift) & mask;
+}
+
+// lanes of the warp holding the same digit (9 bits: SORT_RADIX marks an invalid lane), by one
+// ballot per bit: no MATCH instruction on the critical path
+#ifndef SVF_SORT_USE_MATCH
+#define SVF_SORT_USE_MATCH 0
+#endif
+__device__ __forceinline__ uint32_t warp_match_digit(uint32_t d, bool valid)
+{
+#if SVF_SORT_USE_MATCH
+    return __match_any_sync(0xffffffffu, d);
+#else
+    uint32_t peers = __ballot_sync(0xffffffffu, valid);
+    if (!valid) peers = ~peers;
+#pragma unroll
+    for (int b = 0; b < SORT_RADIX_BITS; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const uint32_t m = __ballot_sync(0xffffffffu, bit);
+        peers &= bit ? m : ~m;
+    }
+    return peers;
+#endif
 }
 
 // ---- histogram of every digit in one read of the input ---------------------------------------
@@ -52,14 +78,23 @@ __global__ void __launch_bounds__(512) k_sort_hist(const uint64_t* __restrict__ 
 #pragma unroll
     for (int p = 0; p < NPASS; ++p) { last[p] = 0; cnt[p] = 0; }
 
+    // four independent loads in flight per thread (the kernel is latency bound otherwise)
+    constexpr int UNR = 4;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        uint64_t w = __ldg(in + i);
+    for (int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < n; i0 += stride * UNR) {
+        uint64_t w[UNR];
 #pragma unroll
-        for (int p = 0; p < NPASS; ++p) {
-            uint32_t d = digit_of(w, shift[p], mask[p]);
-            if (d == last[p]) ++cnt[p];
-            else { if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]); last[p] = d; cnt[p] = 1; }
+        for (int u = 0; u < UNR; ++u) { const int64_t i = i0 + u * stride; w[u] = i < n ? __ldg(in + i) : 0ull; }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            if (i0 + u * stride < n) {
+#pragma unroll
+                for (int p = 0; p < NPASS; ++p) {
+                    uint32_t d = digit_of(w[u], shift[p], mask[p]);
+                    if (d == last[p]) ++cnt[p];
+                    else { if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]); last[p] = d; cnt[p] = 1; }
+                }
+            }
         }
     }
 #pragma unroll
@@ -93,11 +128,17 @@ __global__ void __launch_bounds__(SORT_RADIX) k_sort_plan(uint32_t* __restrict__
         __syncthreads();
     }
     if (tid == 0) {
+        // ping-pong x, y so that the LAST executed pass writes x (the caller's output buffer: no
+        // copy afterwards); when y aliases the input the first pass must write x instead
+        int exec = 0;
+        for (int p = 0; p < npass; ++p) exec += skip_s[p] ? 0 : 1;
+        bool to_x = (y == in) ? true : ((exec & 1) != 0);
         const uint64_t* cur = in;
         for (int p = 0; p < npass; ++p) {
             plan->skip[p] = skip_s[p];
             if (skip_s[p]) { plan->src[p] = nullptr; plan->dst[p] = nullptr; continue; }
-            uint64_t* d = (cur == x) ? y : x;
+            uint64_t* d = to_x ? x : y;
+            to_x = !to_x;
             plan->src[p] = cur; plan->dst[p] = d; cur = d;
         }
         plan->result = cur;
@@ -132,7 +173,7 @@ __device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gsrc, ui
 }
 
 // ---- one onesweep pass -----------------------------------------------------------------------
-__global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __restrict__ plan,
+__global__ void __launch_bounds__(SORT_THREADS, 4) k_sort_pass(const SortPlan* __restrict__ plan,
                                                             int p, int64_t n, int shift,
                                                             uint32_t mask,
                                                             uint32_t* __restrict__ tile_ctr,
@@ -142,6 +183,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __re
     constexpr int WARPS = SORT_THREADS / 32;
     __shared__ __align__(128) uint64_t staging[SORT_TILE];
     __shared__ uint32_t whist[WARPS * SORT_RADIX];
+    __shared__ uint32_t thist[SORT_RADIX];
     __shared__ uint32_t toff_s[SORT_RADIX];
     __shared__ uint32_t gbase_s[SORT_RADIX];
     __shared__ uint32_t warp_tot[SORT_RADIX / 32];
@@ -155,6 +197,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __re
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
     if (tid == 0) { tile_s = atomicAdd(&tile_ctr[p], 1u); mbar_init(&bar, 1); }
     for (int i = tid; i < WARPS * SORT_RADIX; i += SORT_THREADS) whist[i] = 0;
+    thist[tid] = 0;
     __syncthreads();
     const uint32_t tile = tile_s;
     const int64_t tile_base = (int64_t)tile * SORT_TILE;
@@ -181,6 +224,26 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __re
         }
     }
 
+    // the tile's digit counts first (shared-memory atomics), published BEFORE the ranking: the
+    // successors' look-back then finds an aggregate while this tile is still ranking
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i)
+        if ((wbase + i * 32 + lane) < tile_n) atomicAdd(&thist[digit_of(key[i], shift, mask)], 1u);
+    __syncthreads();
+    const uint32_t count = thist[tid];
+    volatile uint32_t* st = status + (size_t)tile * SORT_RADIX + tid;
+    *st = (tile == 0 ? FLAG_INCL : FLAG_AGG) | count;
+    {   // tile-level exclusive scan of the counts
+        uint32_t inc = count;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) warp_tot[wrp] = inc;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
+        toff_s[tid] = off + inc - count;
+    }
+
     // per-warp stable ranking with digit ballots
     uint32_t* wh = whist + wrp * SORT_RADIX;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -189,49 +252,54 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_pass(const SortPlan* __re
     for (int i = 0; i < SORT_IPT; ++i) {
         const bool valid = (wbase + i * 32 + lane) < tile_n;
         const uint32_t d = valid ? digit_of(key[i], shift, mask) : SORT_RADIX;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t peers = warp_match_digit(d, valid);
+        // the highest peer owns the warp-private counter of its digit for this round
+        const int leader = 31 - __clz(peers);
         uint32_t base = 0;
-        if (valid) base = wh[d];
-        __syncwarp();
-        if (valid && lane == (31 - __clz(peers))) wh[d] = base + __popc(peers);
+        if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
+        base = __shfl_sync(0xffffffffu, base, leader);
         __syncwarp();
         rank[i] = base + __popc(peers & lt_mask);
     }
     __syncthreads();
 
-    // digit d (thread d): exclusive scan over warps, tile count, publish, tile-level scan
-    uint32_t count = 0;
+    // digit d (thread d): exclusive scan of the warp-private counts over the warps; then the
+    // decoupled look-back over the predecessor tiles of this digit (their aggregates were
+    // published before their ranking, so this rarely waits)
     {
         uint32_t run = 0;
 #pragma unroll
         for (int w = 0; w < WARPS; ++w) { uint32_t c = whist[w * SORT_RADIX + tid]; whist[w * SORT_RADIX + tid] = run; run += c; }
-        count = run;
-        volatile uint32_t* st = status + (size_t)tile * SORT_RADIX + tid;
-        *st = (tile == 0 ? FLAG_INCL : FLAG_AGG) | count;
-        uint32_t inc = count;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-        if (lane == 31) warp_tot[wrp] = inc;
-        __syncthreads();
-        uint32_t off = 0;
-        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
-        const uint32_t toff = off + inc - count;
-        toff_s[tid] = toff;
-        // decoupled look-back over the predecessor tiles of this digit
         uint32_t excl = 0;
         if (tile > 0) {
+            // eight predecessors per round trip to L2 (independent loads), consumed in order
+            constexpr int LOOK = 8;
             int64_t look = (int64_t)tile - 1;
-            while (true) {
-                uint32_t v = *(volatile uint32_t*)(status + (size_t)look * SORT_RADIX + tid);
-                uint32_t f = v >> 30;
-                if (f == 0) continue;
-                excl += v & VALUE_MASK;
-                if (f == 2) break;
-                --look;
+            bool done = false;
+            while (!done) {
+                uint32_t v[LOOK];
+#pragma unroll
+                for (int q = 0; q < LOOK; ++q) {
+                    const int64_t idx = look - q;
+                    v[q] = idx >= 0 ? *(volatile uint32_t*)(status + (size_t)idx * SORT_RADIX + tid) : (2u << 30);   // past tile 0: an empty inclusive word
+                }
+                int used = 0;
+#pragma unroll
+                for (int q = 0; q < LOOK; ++q) {
+                    if (!done && used == q) {
+                        const uint32_t f = v[q] >> 30;
+                        if (f != 0) {
+                            excl += v[q] & VALUE_MASK;
+                            ++used;
+                            if (f == 2) done = true;
+                        }
+                    }
+                }
+                look -= used;
             }
             *st = FLAG_INCL | (excl + count);
         }
-        gbase_s[tid] = bases[tid] + excl - toff;    // modulo 2^32; dst index = gbase + slot
+        gbase_s[tid] = bases[tid] + excl - toff_s[tid];    // modulo 2^32; dst index = gbase + slot
     }
     __syncthreads();
 
@@ -290,11 +358,11 @@ __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64
         const bool valid = e < n;
         key[i] = valid ? in[e] : 0ull;
         const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & 0xffu) : SORT_RADIX;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t peers = warp_match_digit(d, valid);
+        const int leader = 31 - __clz(peers);
         uint32_t base = 0;
-        if (valid) base = wh[d];
-        __syncwarp();
-        if (valid && lane == (31 - __clz(peers))) wh[d] = base + __popc(peers);
+        if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
+        base = __shfl_sync(0xffffffffu, base, leader);
         __syncwarp();
         rank[i] = base + __popc(peers & lt_mask);
     }
