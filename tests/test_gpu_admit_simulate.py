@@ -128,6 +128,36 @@ def test_config3_full_size_sampled(B, oracle):
     assert not got["status"][:4096].any()
 
 
+def test_bench_launch_configuration_sampled(B, oracle):
+    """The exact call bench.py times: configs[2] at full size, all four policies in ONE
+    svf_simulate_policies launch, every output; 96 sampled instances per policy against the
+    oracle, every field, plus properties that hold at any size for all instances."""
+    import torch
+    tr = T.config3(n_instances=4096, lam=4.0)
+    dt = B.DeviceTrace.from_host(tr)
+    outs = B.svf_simulate_policies(dt, [0, 1, 2, 3])
+    torch.cuda.synchronize()
+    sub = np.arange(5, 4096, 43)
+    subtr = tr.subset(sub)
+    rows = np.concatenate([np.arange(tr.offsets[j], tr.offsets[j + 1]) for j in sub])
+    sum_o = np.add.reduceat(tr.output.astype(np.int64), tr.offsets[:-1])
+    for pol, out in zip(range(4), outs):
+        ref = oracle.simulate(subtr, pol, n_threads=8)
+        for k in FIELDS:
+            g = getattr(out, k).cpu().numpy()
+            g = g[rows] if k in ("start", "finish") else g[sub]
+            assert np.array_equal(g, getattr(ref, k)), f"policy {pol} field {k}"
+        start, finish = out.start.cpu().numpy(), out.finish.cpu().numpy()
+        assert not out.status.cpu().numpy().any()
+        assert np.array_equal(finish - start, tr.output)                     # non-preemptive, o steps each
+        assert (start >= tr.arrival).all()
+        tel = out.total_latency.cpu().numpy()
+        assert np.array_equal(tel, np.add.reduceat((finish - tr.arrival).astype(np.int64), tr.offsets[:-1]))
+        assert (tel >= sum_o).all()                                          # Lemma G.1, P:L485
+        assert (out.peak_kv.cpu().numpy() <= tr.M).all()                     # Eq. 3c
+        assert np.array_equal(out.makespan.cpu().numpy(), np.maximum.reduceat(finish, tr.offsets[:-1]))
+
+
 def test_config4_high_concurrency_reduced(B, oracle):
     """configs[3] laws at n=20,000 (state in the global-memory slot: > 16k entries)."""
     tr = T.config4(n=20_000, M=1_000_000)
