@@ -233,17 +233,22 @@ typedef struct {
     int32_t makespan, status;
 } inst_result_t;
 
+/* okey (may be NULL): PREDICTED output lengths, used for the SVF / SJF priority key only (the
+ * paper's deployable SVF / SJF; NULL = the true lengths = "Oracle SVF / SJF").
+ * Dynamics and the feasibility check always use the true o (reading R7). */
+static int64_t key_len(const int32_t *o, const int32_t *okey, int64_t i) { return okey ? okey[i] : o[i]; }
+
 static int32_t validate_instance(int policy, int64_t n, const int32_t *a, const int32_t *s,
-                                 const int32_t *o, const uint8_t *bit, int64_t O0, int64_t O1,
-                                 int64_t M)
+                                 const int32_t *o, const int32_t *okey, const uint8_t *bit,
+                                 int64_t O0, int64_t O1, int64_t M)
 {
     int range = 0, unsorted = 0, infeasible = 0, overflow = 0;
     int64_t sum_o = 0, max_a = 0;
     for (int64_t i = 0; i < n; ++i) {
-        if (o[i] < 1 || s[i] < 0 || a[i] < 0) range = 1;
+        if (o[i] < 1 || s[i] < 0 || a[i] < 0 || (okey && okey[i] < 1)) range = 1;
         if (i > 0 && a[i] < a[i - 1]) unsorted = 1;
         if ((int64_t)s[i] + o[i] > M) infeasible = 1;
-        if (ref_key(policy, s[i], o[i], a[i], bit ? bit[i] : 0, O0, O1) >= ((int64_t)1 << 32))
+        if (ref_key(policy, s[i], key_len(o, okey, i), a[i], bit ? bit[i] : 0, O0, O1) >= ((int64_t)1 << 32))
             overflow = 1;
         sum_o += o[i] > 0 ? o[i] : 0;
         if (a[i] > max_a) max_a = a[i];
@@ -258,12 +263,12 @@ static int32_t validate_instance(int policy, int64_t n, const int32_t *a, const 
 
 static void simulate_instance(int policy, int64_t M, int feas_mode, int64_t n,
                               const int32_t *a, const int32_t *s, const int32_t *o,
-                              const uint8_t *bit, int64_t O0, int64_t O1,
+                              const int32_t *okey, const uint8_t *bit, int64_t O0, int64_t O1,
                               int32_t *start, int32_t *finish, inst_result_t *res)
 {
     memset(res, 0, sizeof(*res));
     for (int64_t i = 0; i < n; ++i) { if (start) start[i] = -1; if (finish) finish[i] = -1; }
-    res->status = validate_instance(policy, n, a, s, o, bit, O0, O1, M);
+    res->status = validate_instance(policy, n, a, s, o, okey, bit, O0, O1, M);
     if (res->status != ST_OK || n == 0) return;
 
     int32_t *k = (int32_t *)malloc(sizeof(int32_t) * (size_t)n);      /* start times k_i */
@@ -291,7 +296,7 @@ static void simulate_instance(int policy, int64_t M, int feas_mode, int64_t n,
         while (next_arrival < n && a[next_arrival] <= t) {
             int32_t i = (int32_t)next_arrival++;
             waiter_t x;
-            x.key = ref_key(policy, s[i], o[i], a[i], bit ? bit[i] : 0, O0, O1);
+            x.key = ref_key(policy, s[i], key_len(o, okey, i), a[i], bit ? bit[i] : 0, O0, O1);
             x.arrival = a[i]; x.id = i;
             int64_t lo = 0, hi = n_wait;              /* first position whose waiter < x */
             while (lo < hi) {
@@ -357,12 +362,13 @@ static void simulate_instance(int policy, int64_t M, int feas_mode, int64_t n,
  * threads when built with OpenMP; each instance itself is one serial step chain).
  * Any output pointer may be NULL.
  * ---------------------------------------------------------------------------------------- */
-int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t *arrival,
-                     const int32_t *prompt, const int32_t *output, const uint8_t *bit,
-                     int32_t O0, int32_t O1, int policy, int64_t M, int feas_mode, int n_threads,
-                     int32_t *start, int32_t *finish, int64_t *total_latency,
-                     int64_t *p99_latency, int32_t *makespan, int64_t *peak_kv, int64_t *rounds,
-                     int64_t *decisions, int32_t *status)
+int svf_ref_simulate_pred(int64_t n_instances, const int64_t *offsets, const int32_t *arrival,
+                          const int32_t *prompt, const int32_t *output, const int32_t *output_key,
+                          const uint8_t *bit, int32_t O0, int32_t O1, int policy, int64_t M,
+                          int feas_mode, int n_threads,
+                          int32_t *start, int32_t *finish, int64_t *total_latency,
+                          int64_t *p99_latency, int32_t *makespan, int64_t *peak_kv, int64_t *rounds,
+                          int64_t *decisions, int32_t *status)
 {
     if (n_instances < 0 || policy < 0 || policy > 3 || M < 0) return ST_EINVAL;
     if (policy == POL_SVF_1BIT && (!bit || O0 < 1 || O1 < 1)) return ST_EINVAL;
@@ -374,6 +380,7 @@ int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t 
         int64_t lo = offsets[j], n = offsets[j + 1] - offsets[j];
         inst_result_t r;
         simulate_instance(policy, M, feas_mode, n, arrival + lo, prompt + lo, output + lo,
+                          output_key ? output_key + lo : NULL,
                           bit ? bit + lo : NULL, O0, O1, start ? start + lo : NULL,
                           finish ? finish + lo : NULL, &r);
         if (total_latency) total_latency[j] = r.total_latency;
@@ -385,6 +392,18 @@ int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t 
         if (status) status[j] = r.status;
     }
     return ST_OK;
+}
+
+int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t *arrival,
+                     const int32_t *prompt, const int32_t *output, const uint8_t *bit,
+                     int32_t O0, int32_t O1, int policy, int64_t M, int feas_mode, int n_threads,
+                     int32_t *start, int32_t *finish, int64_t *total_latency,
+                     int64_t *p99_latency, int32_t *makespan, int64_t *peak_kv, int64_t *rounds,
+                     int64_t *decisions, int32_t *status)
+{
+    return svf_ref_simulate_pred(n_instances, offsets, arrival, prompt, output, NULL, bit, O0, O1, policy, M,
+                                 feas_mode, n_threads, start, finish, total_latency, p99_latency, makespan,
+                                 peak_kv, rounds, decisions, status);
 }
 
 int svf_ref_max_threads(void)

@@ -111,8 +111,13 @@ class SimResult:
     status: np.ndarray
 
 
-def simulate(trace, policy, M=None, mode=FEAS_COMPLETION, n_threads=1) -> SimResult:
-    """Run the time-stepped simulator on every instance of ``trace`` (a traces.Trace)."""
+def simulate(trace, policy, M=None, mode=FEAS_COMPLETION, n_threads=1, output_key="trace") -> SimResult:
+    """Run the time-stepped simulator on every instance of ``trace`` (a traces.Trace).
+    ``output_key``: predicted output lengths used for the SVF / SJF key only (default: the
+    trace's own ``output_key`` if it has one; None = the true lengths)."""
+    if isinstance(output_key, str):
+        output_key = getattr(trace, "output_key", None)
+    ok = _i32(output_key)
     M = trace.M if M is None else M
     I, N = trace.n_instances, trace.n_requests
     off = np.ascontiguousarray(trace.offsets, dtype=np.int64)
@@ -120,9 +125,9 @@ def simulate(trace, policy, M=None, mode=FEAS_COMPLETION, n_threads=1) -> SimRes
     r = SimResult(np.full(N, -1, np.int32), np.full(N, -1, np.int32), np.zeros(I, np.int64),
                   np.zeros(I, np.int64), np.zeros(I, np.int32), np.zeros(I, np.int64),
                   np.zeros(I, np.int64), np.zeros(I, np.int64), np.zeros(I, np.int32))
-    rc = lib().svf_ref_simulate(
+    rc = lib().svf_ref_simulate_pred(
         C.c_int64(I), _p(off, C.c_int64), _p(a, C.c_int32), _p(s, C.c_int32), _p(o, C.c_int32),
-        _p(b, C.c_uint8), C.c_int32(trace.O0), C.c_int32(trace.O1), C.c_int(policy),
+        _p(ok, C.c_int32), _p(b, C.c_uint8), C.c_int32(trace.O0), C.c_int32(trace.O1), C.c_int(policy),
         C.c_int64(M), C.c_int(mode), C.c_int(n_threads),
         _p(r.start, C.c_int32), _p(r.finish, C.c_int32), _p(r.total_latency, C.c_int64),
         _p(r.p99_latency, C.c_int64), _p(r.makespan, C.c_int32), _p(r.peak_kv, C.c_int64),

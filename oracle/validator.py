@@ -74,7 +74,10 @@ def validate(trace, policy, start, M=None, finish=None, check_blocked="all", max
     vol = s * o + (o * (o + 1)) // 2
     assert int(mem.sum()) == int(vol.sum()), "area conservation violated"
     # (iv) prefix property
-    key = priority_keys(policy, a, s, o, trace.bit, trace.O0, trace.O1)
+    # the ORDER may come from predicted lengths (trace.output_key); dynamics use the true o
+    okey = getattr(trace, "output_key", None)
+    o_for_key = o if okey is None else np.asarray(okey, dtype=np.int64)
+    key = priority_keys(policy, a, s, o_for_key, trace.bit, trace.O0, trace.O1)
     order = np.lexsort((np.arange(n), a, key))          # ascending (key, arrival, id)
     pos = np.empty(n, dtype=np.int64)
     pos[order] = np.arange(n)

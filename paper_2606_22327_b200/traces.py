@@ -107,6 +107,7 @@ class Trace:
     O0: int
     O1: int
     meta: dict = field(default_factory=dict)
+    output_key: np.ndarray = None   # int32 [N] predicted output lengths (key only) or None
 
     @property
     def n_instances(self) -> int:
@@ -130,7 +131,8 @@ class Trace:
         return Trace(f"{self.name}[{j}]", np.array([0, hi - lo], dtype=np.int64),
                      self.arrival[lo:hi].copy(), self.prompt[lo:hi].copy(),
                      self.output[lo:hi].copy(), self.bit[lo:hi].copy(), self.M, self.O0, self.O1,
-                     dict(self.meta))
+                     dict(self.meta),
+                     None if self.output_key is None else self.output_key[lo:hi].copy())
 
     def subset(self, idx) -> "Trace":
         parts = [self.instance(int(j)) for j in idx]
@@ -157,8 +159,11 @@ def concat(parts, name, M, O0, O1, meta=None) -> Trace:
     offsets[1:] = np.cumsum(sizes)
     cat = lambda key, dt: (np.concatenate([getattr(p, key) for p in parts]).astype(dt)
                            if parts else np.zeros(0, dt))
+    okey = None
+    if parts and all(p.output_key is not None for p in parts):
+        okey = cat("output_key", np.int32)
     return Trace(name, offsets, cat("arrival", np.int32), cat("prompt", np.int32),
-                 cat("output", np.int32), cat("bit", np.uint8), M, O0, O1, meta or {})
+                 cat("output", np.int32), cat("bit", np.uint8), M, O0, O1, meta or {}, okey)
 
 
 def _one(name, a, s, o, bit, M, O0, O1, meta=None) -> Trace:
@@ -269,3 +274,20 @@ def random_small(seed: int, n: int, s_hi: int, o_hi: int, M: int, a_hi: int = 0,
     a = np.sort(uniform_int(sd, _ST_GAP, n, 0, a_hi)) if a_hi > 0 else np.zeros(n, np.int32)
     bit = (uniform(sd, _ST_FLIP, n) < 0.5).astype(np.uint8)
     return _one(f"rand[{seed}]", a, s, o, bit, M, O0, O1, {"burst": a_hi == 0})
+
+
+# ---------------------------------------------------------------------------------------------
+# Predicted output lengths: a stand-in for the paper's BERT length predictor
+# (PAPER.md:215), which needs prompts and trained weights that are not available here
+# ---------------------------------------------------------------------------------------------
+def with_predicted_lengths(trace: Trace, sigma: float = 0.5, seed: int = 0, hi: int = 1 << 20) -> Trace:
+    """A copy of ``trace`` with ``output_key[i] = clip(rint(o_i * exp(sigma * z_i)), 1, hi)``,
+    z_i standard normal from the counter-based generator: multiplicative lognormal prediction
+    noise (sigma = 0 reproduces the true lengths).  Only the ORDER of SVF / SJF sees it."""
+    sd = instance_seed(77, seed)
+    n = trace.n_requests
+    z = normal(sd, _ST_O1, _ST_O2, n)
+    ok = np.clip(np.rint(trace.output.astype(np.float64) * np.exp(sigma * z)), 1, hi).astype(np.int32)
+    return Trace(trace.name + f"[pred sigma={sigma:g}]", trace.offsets.copy(), trace.arrival.copy(),
+                 trace.prompt.copy(), trace.output.copy(), trace.bit.copy(), trace.M, trace.O0, trace.O1,
+                 dict(trace.meta), ok)

@@ -262,3 +262,63 @@ def test_admit_matches_simulator_first_step(oracle):
             rc2, idx2, _ = oracle.admit(policy, tr.M, 0, tr.prompt, tr.output, tr.arrival,
                                         tr.bit, tr.O0, tr.O1, [], [], mode=0)
             assert np.array_equal(idx, idx2)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: predicted output lengths order the queue, true lengths drive the model
+# (deployable SVF / SJF vs Oracle-SVF / Oracle-SJF; reading R7)
+# ---------------------------------------------------------------------------------------------
+def test_predicted_keys_equal_to_true_lengths_change_nothing(oracle):
+    tr = T.config3(n_instances=6, n=150, lam=4.0, M=40_000)
+    same = T.with_predicted_lengths(tr, sigma=0.0)
+    assert np.array_equal(same.output_key, tr.output)
+    for policy in range(4):
+        a, b = oracle.simulate(tr, policy), oracle.simulate(same, policy)
+        assert np.array_equal(a.start, b.start) and np.array_equal(a.total_latency, b.total_latency)
+
+
+def test_predicted_keys_hand_example(oracle):
+    """Hand example A (tests/golden/hand_examples.txt: M=8, (s,o) = (2,3), (1,2), (3,1), burst).
+    True SJF admits r2, r1 first: TEL 7.  With predictions (1, 2, 3) SJF's order is r0, r1, r2, the
+    FCFS order, so by Eq. 3c: r0, r1 start at 0; r2 is blocked at t=0,1,2 (mem 9, 11, 9 > 8) and
+    starts at 3: TEL = 3 + 2 + 4 = 9 -- the schedule derived by hand for FCFS."""
+    tr = T._one("exA", np.zeros(3, np.int32), np.array([2, 1, 3]), np.array([3, 2, 1]), np.zeros(3, np.uint8), 8, 1, 1)
+    true_sjf = oracle.simulate(tr, oracle.SJF)
+    assert list(true_sjf.start) == [1, 0, 0] and int(true_sjf.total_latency[0]) == 7
+    tr.output_key = np.array([1, 2, 3], np.int32)
+    for mode in (oracle.FEAS_LITERAL, oracle.FEAS_COMPLETION):
+        r = oracle.simulate(tr, oracle.SJF, mode=mode)
+        assert list(r.start) == [0, 0, 3] and list(r.finish) == [3, 2, 4] and int(r.total_latency[0]) == 9
+    # the true lengths still drive the dynamics: finish - start is the TRUE o
+    assert np.array_equal(r.finish - r.start, tr.output)
+
+
+def test_constant_prediction_orders_svf_by_prompt_like_equal_bits(oracle):
+    """If every prediction is the same length c, Eq. 1 with o := c is s*c + c(c+1)/2: the order is
+    by s, exactly what 1-bit SVF (Eq. 2) gives when every bit is 0 and O_0 = c -- a different key
+    routine of the oracle reaching the same schedule."""
+    for seed in range(6):
+        tr = T.random_small(400 + seed, 40, 9, 11, 30, a_hi=25, O0=5, O1=9)
+        tr.bit[:] = 0
+        one_bit = oracle.simulate(tr, oracle.SVF_1BIT)
+        tr.output_key = np.full(tr.n_requests, 5, np.int32)
+        pred = oracle.simulate(tr, oracle.SVF)
+        assert np.array_equal(pred.start, one_bit.start)
+        # FCFS and 1-bit SVF never look at the predictions
+        for policy in (oracle.SVF_1BIT, oracle.FCFS):
+            assert np.array_equal(oracle.simulate(tr, policy).start, oracle.simulate(tr, policy, output_key=None).start)
+
+
+@pytest.mark.parametrize("policy", [0, 2])
+def test_predicted_keys_schedules_pass_the_validator(oracle, policy):
+    """Noisy predictions: the schedule is still feasible, non-preemptive, greedy in the PREDICTED
+    order with no bypass (validator (i)-(iv)), and latency >= true o."""
+    from oracle import validator
+    for seed in range(4):
+        tr = T.with_predicted_lengths(T.random_small(500 + seed, 50, 9, 11, 26, a_hi=30), sigma=0.9, seed=seed, hi=40)
+        r = oracle.simulate(tr, policy)
+        facts = validator.validate(tr, policy, r.start, finish=r.finish)
+        assert facts["peak_kv"] <= tr.M and facts["total_latency"] == int(r.total_latency[0])
+    bad = T.with_predicted_lengths(T.random_small(1, 10, 9, 11, 26), sigma=0.5)
+    bad.output_key[3] = 0
+    assert int(oracle.simulate(bad, policy).status[0]) == oracle.ERANGE
