@@ -65,6 +65,11 @@ typedef struct {
     const int32_t* output;        /* [dev] [N] o_i >= 1 (true length: drives dynamics AND the check, R7) */
     const uint8_t* bit;           /* [dev] [N] 0 = short, 1 = long; may be NULL unless SVF_SVF_1BIT */
     int32_t        O0, O1;        /* [host] integer proxy lengths of Eq. 2 (>= 1 for SVF_SVF_1BIT)   */
+    const int32_t* output_key;    /* [dev] [N] or NULL: PREDICTED output lengths (>= 1) that replace
+                                     o_i in the SVF (Eq. 1) and SJF keys only -- the deployable
+                                     SVF / SJF of the paper; NULL = true lengths =
+                                     "Oracle-SVF / Oracle-SJF".  Dynamics and the check
+                                     always use `output` (R7).                                      */
 } svf_trace_t;
 
 /* Caller-allocated DEVICE outputs of svf_simulate.  Any pointer may be NULL (not wanted). */

@@ -37,7 +37,8 @@ class SvfError(RuntimeError):
 class _Trace(C.Structure):
     _fields_ = [("n_instances", C.c_int64), ("n_requests", C.c_int64), ("max_instance", C.c_int64),
                 ("offsets", C.c_void_p), ("arrival", C.c_void_p), ("prompt", C.c_void_p),
-                ("output", C.c_void_p), ("bit", C.c_void_p), ("O0", C.c_int32), ("O1", C.c_int32)]
+                ("output", C.c_void_p), ("bit", C.c_void_p), ("O0", C.c_int32), ("O1", C.c_int32),
+                ("output_key", C.c_void_p)]
 
 
 class _Result(C.Structure):
@@ -243,6 +244,7 @@ class DeviceTrace:
     O0: int
     O1: int
     M: int
+    output_key: Optional[torch.Tensor] = None   # int32 [N] predicted lengths (SVF / SJF key only)
 
     @staticmethod
     def from_host(trace, device="cuda", pinned=None, non_blocking=False) -> "DeviceTrace":
@@ -254,7 +256,9 @@ class DeviceTrace:
         return DeviceTrace(up("offsets", trace.offsets, torch.int64), up("arrival", trace.arrival, torch.int32),
                            up("prompt", trace.prompt, torch.int32), up("output", trace.output, torch.int32),
                            up("bit", trace.bit, torch.uint8), trace.n_instances, trace.n_requests,
-                           trace.max_n, int(trace.O0), int(trace.O1), int(trace.M))
+                           trace.max_n, int(trace.O0), int(trace.O1), int(trace.M),
+                           None if getattr(trace, "output_key", None) is None
+                           else torch.from_numpy(trace.output_key).to(device=device, dtype=torch.int32))
 
     def nbytes(self) -> int:
         return sum(int(t.numel() * t.element_size()) for t in
@@ -264,7 +268,8 @@ class DeviceTrace:
         return _Trace(self.n_instances, self.n_requests, self.max_instance,
                       self.offsets.data_ptr(), self.arrival.data_ptr(), self.prompt.data_ptr(),
                       self.output.data_ptr(), self.bit.data_ptr() if self.bit is not None else None,
-                      self.O0, self.O1)
+                      self.O0, self.O1,
+                      self.output_key.data_ptr() if self.output_key is not None else None)
 
 
 RESULT_FIELDS = ("start", "finish", "total_latency", "p99_latency", "makespan", "peak_kv", "rounds",

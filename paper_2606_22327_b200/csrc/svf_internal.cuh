@@ -92,8 +92,9 @@ int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int6
 // the (s, o, id, a) records in priority order.  One launch.
 constexpr int SEG_SORT_MAX = 4096;
 int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
-                  const int32_t* s, const int32_t* o, const int32_t* a, const uint8_t* bit, int32_t O0,
-                  int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st, int64_t* launches);
+                  const int32_t* s, const int32_t* o, const int32_t* okey /* key lengths or NULL */,
+                  const int32_t* a, const uint8_t* bit, int32_t O0, int32_t O1, uint32_t* order, uint32_t* rank,
+                  int4* req, cudaStream_t st, int64_t* launches);
 // copy plan->result to out unless it already is out
 int sort_result_to(const SortWs& w, uint64_t* out, int64_t n, cudaStream_t st, int64_t* launches);
 

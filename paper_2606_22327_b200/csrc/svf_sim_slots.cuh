@@ -134,6 +134,7 @@ struct SlotArgs {
     int32_t O0, O1;
     const int64_t* off;
     const int32_t *a, *s, *o;
+    const int32_t* okey;             // [N] predicted lengths for the SVF / SJF key, or NULL
     const uint8_t* bit;
     int n_policies;
     PolicyIO io[MAX_POLICIES];
@@ -306,11 +307,12 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         int max_a = 0;
         for (int i = tid; i < n; i += THREADS) {
             const int32_t ai = a[i], si = s[i], oi = o[i];
-            if (oi < 1 || si < 0 || ai < 0) flags |= F_RANGE;
+            const int32_t ki = g.okey ? g.okey[base + i] : oi;      // length the key sees
+            if (oi < 1 || si < 0 || ai < 0 || ki < 1) flags |= F_RANGE;
             if (i > 0 && ai < a[i - 1]) flags |= F_UNSORTED;
             if ((int64_t)si + oi > g.M) flags |= F_INFEASIBLE;
             const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
-            if (oi >= 1 && si >= 0 && ai >= 0 && (priority_key(policy, si, oi, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
+            if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
             max_a = ai > max_a ? ai : max_a;
         }

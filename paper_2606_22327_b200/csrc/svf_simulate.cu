@@ -32,6 +32,7 @@ struct SimArgs {
     int sb;                          // bits of the local-id field
     const int64_t* off;
     const int32_t *a, *s, *o;
+    const int32_t* okey;             // [N] predicted lengths for the SVF / SJF key, or NULL
     const uint8_t* bit;
     const uint32_t* order;           // [N] local id at (instance offset + rank)
     const uint32_t* rank;            // [N] rank of (instance offset + local id)
@@ -67,7 +68,7 @@ __global__ void __launch_bounds__(256) k_sim_pack(SimArgs g, uint64_t* __restric
         }
         const int64_t seq = i - __ldg(g.off + lo);
         const uint32_t b = g.policy == SVF_SVF_1BIT ? (uint32_t)__ldg(g.bit + i) : 0u;
-        const uint64_t key = priority_key(g.policy, __ldg(g.s + i), __ldg(g.o + i), __ldg(g.a + i), b, g.O0, g.O1);
+        const uint64_t key = priority_key(g.policy, __ldg(g.s + i), __ldg((g.okey ? g.okey : g.o) + i), __ldg(g.a + i), b, g.O0, g.O1);
         words[i] = ((uint64_t)lo << (32 + g.sb)) | ((key & 0xffffffffull) << g.sb) | ((uint64_t)seq & seq_mask);
     }
 }
@@ -136,11 +137,12 @@ __global__ void __launch_bounds__(THREADS) k_sim(SimArgs g)
         int max_a = 0;
         for (int i = tid; i < n; i += THREADS) {
             const int32_t ai = a[i], si = s[i], oi = o[i];
-            if (oi < 1 || si < 0 || ai < 0) flags |= F_RANGE;
+            const int32_t ki = g.okey ? g.okey[base + i] : oi;      // length the key sees
+            if (oi < 1 || si < 0 || ai < 0 || ki < 1) flags |= F_RANGE;
             if (i > 0 && ai < a[i - 1]) flags |= F_UNSORTED;
             if ((int64_t)si + oi > g.M) flags |= F_INFEASIBLE;
             const uint32_t b = g.policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
-            if (oi >= 1 && si >= 0 && ai >= 0 && (priority_key(g.policy, si, oi, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
+            if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(g.policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
             max_a = ai > max_a ? ai : max_a;
         }
@@ -503,7 +505,7 @@ int simulate_wide(const svf_trace_t* tr, int policy, int64_t M, const svf_result
     SimArgs g;
     g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
     g.policy = policy; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
-    g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
+    g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.okey = tr->output_key; g.bit = tr->bit;
     g.order = w.order[0]; g.rank = w.rank[0]; g.req = w.req[0];
     g.start = out->start; g.finish = out->finish; g.tel = out->total_latency; g.peak = out->peak_kv;
     g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
@@ -593,7 +595,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     SlotArgs q;
     q.I = I; q.N = N; q.M = M; q.max_instance = tr->max_instance;
     q.O0 = tr->O0; q.O1 = tr->O1;
-    q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.bit = tr->bit;
+    q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.okey = tr->output_key; q.bit = tr->bit;
     q.n_policies = P;
     if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
     for (int k = 0; k < P; ++k) {
@@ -608,7 +610,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
         io.lat = w.lat[k];
         if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
             // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance
-            if (seg_sort_keys(policies[k], I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->arrival,
+            if (seg_sort_keys(policies[k], I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->output_key, tr->arrival,
                               tr->bit, tr->O0, tr->O1, w.order[k], w.rank[k], c.qreg ? nullptr : w.req[k], st,
                               &g_launches_sim))
                 return SVF_ECUDA;
@@ -616,7 +618,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
             SimArgs g;
             g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
             g.policy = policies[k]; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
-            g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.bit = tr->bit;
+            g.off = tr->offsets; g.a = tr->arrival; g.s = tr->prompt; g.o = tr->output; g.okey = tr->output_key; g.bit = tr->bit;
             g.req = c.qreg ? nullptr : w.req[k];
             int64_t blocks = ceil_div(N, 256);
             const int64_t capb = (int64_t)sm_count() * 8;

@@ -400,6 +400,7 @@ __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64
 __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I, int64_t N, int cap,
                                                            const int64_t* __restrict__ off,
                                                            const int32_t* __restrict__ s, const int32_t* __restrict__ o,
+                                                           const int32_t* __restrict__ okey,
                                                            const int32_t* __restrict__ a, const uint8_t* __restrict__ bit,
                                                            int32_t O0, int32_t O1, uint32_t* __restrict__ order,
                                                            uint32_t* __restrict__ rank, int4* __restrict__ req)
@@ -423,7 +424,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I
         uint32_t kor = 0;
         for (int i = tid; i < n; i += SORT_THREADS) {
             const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)bit[base + i] : 0u;
-            const uint32_t key = (uint32_t)priority_key(policy, s[base + i], o[base + i], a[base + i], b, O0, O1);
+            const uint32_t key = (uint32_t)priority_key(policy, s[base + i], (okey ? okey : o)[base + i], a[base + i], b, O0, O1);
             buf0[i] = ((uint64_t)key << 32) | (uint32_t)i;
             kor |= key;
         }
@@ -532,8 +533,9 @@ int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int6
 }
 
 int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
-                  const int32_t* s, const int32_t* o, const int32_t* a, const uint8_t* bit, int32_t O0,
-                  int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st, int64_t* launches)
+                  const int32_t* s, const int32_t* o, const int32_t* okey, const int32_t* a, const uint8_t* bit,
+                  int32_t O0, int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st,
+                  int64_t* launches)
 {
     if (I <= 0 || N <= 0) return 0;
     if (max_instance > SEG_SORT_MAX) return (int)cudaErrorInvalidValue;
@@ -549,7 +551,7 @@ int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const 
         per_sm = 1;
     int64_t grid = (int64_t)per_sm * sm_count();
     if (grid > I) grid = I;
-    k_seg_sort<<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, a, bit, O0, O1, order, rank, req);
+    k_seg_sort<<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, okey, a, bit, O0, O1, order, rank, req);
     ++*launches;
     return (int)cudaGetLastError();
 }

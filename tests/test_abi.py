@@ -72,7 +72,7 @@ def test_simulate_rejects_bad_host_arguments(svf_lib):
     L.svf_simulate.restype = C.c_int
     L.svf_simulate.argtypes = [C.POINTER(_Trace), C.c_int, C.c_int64, C.POINTER(_Result), C.c_void_p,
                                C.c_size_t, C.c_void_p]
-    tr = _Trace(1, 4, 4, None, None, None, None, None, 1, 1)
+    tr = _Trace(1, 4, 4, None, None, None, None, None, 1, 1, None)
     res = _Result()
     assert L.svf_simulate(None, 0, 10, C.byref(res), None, 0, None) == 1
     assert L.svf_simulate(C.byref(tr), 9, 10, C.byref(res), None, 0, None) == 1           # policy

@@ -265,6 +265,30 @@ def test_policies_call_with_rejected_and_empty_instances(B, oracle):
     assert int(outs[0].status[2]) != 0
 
 
+@pytest.mark.parametrize("sigma", [0.3, 1.0])
+def test_predicted_length_keys(B, oracle, sigma):
+    """NEXT-1: `output_key` (predicted lengths) orders SVF / SJF, the true lengths drive the model
+    (R7).  Every presort path: shared-memory segment sort (warp kernel and CTA
+    kernel), device-wide onesweep (instances > 4096), wide kernel (M >= 2^30)."""
+    cases = [(T.config3(n_instances=64, n=300, lam=4.0, M=60_000), None),
+             (T.config3(n_instances=5, n=1500, lam=8.0, M=60_000), None),
+             (T.config3(n_instances=2, n=6000, lam=8.0, M=60_000), None),
+             (T.config3(n_instances=12, n=100, lam=4.0), 1 << 30)]
+    for base_tr, M in cases:
+        tr = T.with_predicted_lengths(base_tr, sigma=sigma, seed=3, hi=4096)
+        assert not np.array_equal(tr.output_key, tr.output)
+        for policy in range(4):
+            check(B, oracle, tr, policy, M=M, ctx=f"{tr.name} policy {policy}")
+    # predictions change the SVF schedule, but not FCFS
+    tr = T.with_predicted_lengths(cases[0][0], sigma=1.0, seed=3, hi=4096)
+    assert not np.array_equal(run_gpu(B, tr, 0)["start"], run_gpu(B, cases[0][0], 0)["start"])
+    assert np.array_equal(run_gpu(B, tr, 3)["start"], run_gpu(B, cases[0][0], 3)["start"])
+    # a prediction < 1 is a range error of that instance only
+    tr.output_key[tr.offsets[2] + 5] = 0
+    ref, got = check(B, oracle, tr, 0)
+    assert got["status"][2] == oracle.ERANGE and not got["status"][:2].any()
+
+
 def test_outputs_are_optional(B, oracle):
     tr = T.config3(n_instances=8, lam=4.0)
     ref = oracle.simulate(tr, 0)
