@@ -338,7 +338,7 @@ __global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan-
 // rank[] (rank of id) and, if wanted, the (s, o, id, a) records in priority order.  HBM traffic:
 // 12-13 B read + 8 B (24 B with records) written per request, against 8 + 16 B per executed pass
 // of the device-wide sort.
-template <int THREADS>
+template <int THREADS, int IPT>
 __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out, int n, int ipt,
                                          int shift, uint32_t* whist, uint32_t* toff_s, uint32_t* warp_tot)
 {
@@ -349,16 +349,16 @@ __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64
     const int wbase = wrp * 32 * ipt;
     uint32_t* wh = whist + wrp * SORT_RADIX;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    uint64_t key[SORT_IPT];
-    uint32_t rank[SORT_IPT];
+    uint64_t key[IPT];            // IPT >= ipt: sized by the template so small segments stay cheap in registers
+    uint32_t rank[IPT];
 #pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
+    for (int i = 0; i < IPT; ++i) {
         if (i >= ipt) break;                                   // uniform
         const int e = wbase + i * 32 + lane;
         const bool valid = e < n;
         key[i] = valid ? in[e] : 0ull;
         const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & 0xffu) : SORT_RADIX;
-        const uint32_t peers = warp_match_digit(d, valid);
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);   // one segment per CTA: latency matters, not issue slots
         const int leader = 31 - __clz(peers);
         uint32_t base = 0;
         if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
@@ -387,7 +387,7 @@ __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64
     }
     __syncthreads();
 #pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
+    for (int i = 0; i < IPT; ++i) {
         if (i >= ipt) break;
         if (wbase + i * 32 + lane < n) {
             const uint32_t d = (uint32_t)(key[i] >> shift) & 0xffu;
@@ -397,6 +397,7 @@ __device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64
     __syncthreads();
 }
 
+template <int IPT>
 __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I, int64_t N, int cap,
                                                            const int64_t* __restrict__ off,
                                                            const int32_t* __restrict__ s, const int32_t* __restrict__ o,
@@ -436,7 +437,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I
         const int npass = (bits + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
         const int ipt = (n + SORT_THREADS - 1) / SORT_THREADS;
         for (int p = 0; p < npass; ++p) {
-            seg_pass<SORT_THREADS>(buf0, buf1, n, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
+            seg_pass<SORT_THREADS, IPT>(buf0, buf1, n, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
             uint64_t* t = buf0; buf0 = buf1; buf1 = t;
         }
         for (int p = tid; p < n; p += SORT_THREADS) {
@@ -541,17 +542,28 @@ int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const 
     if (max_instance > SEG_SORT_MAX) return (int)cudaErrorInvalidValue;
     const int cap = (int)((max_instance > 0 ? max_instance : 1) + 1) / 2 * 2;
     const size_t smem = (size_t)2 * cap * sizeof(uint64_t);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_seg_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * SEG_SORT_MAX * (int)sizeof(uint64_t));
-        attr_set = true;
-    }
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort, SORT_THREADS, smem) != cudaSuccess || per_sm < 1)
-        per_sm = 1;
-    int64_t grid = (int64_t)per_sm * sm_count();
-    if (grid > I) grid = I;
-    k_seg_sort<<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, okey, a, bit, O0, O1, order, rank, req);
+    // items per thread sized to the largest instance (registers: occupancy of small segments)
+#define SVF_SEG_LAUNCH(IPT)                                                                             \
+    do {                                                                                                \
+        static bool attr_set = false;                                                                   \
+        if (!attr_set) {                                                                                \
+            cudaFuncSetAttribute(k_seg_sort<IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
+                                 2 * SEG_SORT_MAX * (int)sizeof(uint64_t));                             \
+            attr_set = true;                                                                            \
+        }                                                                                               \
+        int per_sm = 0;                                                                                 \
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort<IPT>, SORT_THREADS, smem) \
+                != cudaSuccess || per_sm < 1)                                                           \
+            per_sm = 1;                                                                                 \
+        int64_t grid = (int64_t)per_sm * sm_count();                                                    \
+        if (grid > I) grid = I;                                                                         \
+        k_seg_sort<IPT><<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, okey, \
+                                                                    a, bit, O0, O1, order, rank, req);  \
+    } while (0)
+    if (cap <= 4 * SORT_THREADS) SVF_SEG_LAUNCH(4);
+    else if (cap <= 8 * SORT_THREADS) SVF_SEG_LAUNCH(8);
+    else SVF_SEG_LAUNCH(16);
+#undef SVF_SEG_LAUNCH
     ++*launches;
     return (int)cudaGetLastError();
 }
