@@ -49,8 +49,8 @@ OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
 # start, finish (8) + latency for the p99 selection (4 written, 4 read back)
 SIM_BYTES_PER_REQUEST = 36
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/r01_kslots_full.md
-SIM_DRAM_TRAFFIC_BYTES = 175.7e6
+# `ncu --set full` capture summarised in profiles/r01_kslots_full.md (one launch = four policies)
+SIM_DRAM_TRAFFIC_BYTES = 492.0e6
 
 
 def parse_args():

@@ -14,15 +14,18 @@
 // tid); the rest (only when more than THREADS*K requests run at once) sit in an `ext` array
 // that is only ever touched by the owning thread.
 //
-// Per slot the EVALUATION pass costs six integer instructions:
+// ONE PASS per evaluation, straight-line code, per slot (compile-time register index):
 //     x = f - (t+1)            as unsigned: x < 2^31 iff the slot is live (f > t)
 //     in = x <u o_h            live and f <= f_h            (condition (2) applies)
 //     ge = f >= f_h            (a dead slot has f <= t < f_h)
-//     if (ge) acc += c + f_h   one IADD3                    (condition (1))
+//     if (ge) acc += c + f_h                                (condition (1))
 //     if (in) viol = max(viol, B + (s_h - t - M))           one VIADDMNMX
+//     if (in) B += s_h - t + f                              the admission update, SPECULATIVELY
 //     dead-bit of x shifted into a mask                     (free-slot search, one SHF)
-// the UPDATE pass three (x, in, B += s_h - t + f), and a BLOCKED head costs one more pass that
-// finds how long it must stay blocked (below).  One reduction round per pass.
+// about 6.5 alu-pipe + 2 fma-pipe instructions; then one round of three warp reductions (sum,
+// max, min).  If the head is admitted the update is already in place and the head is written into
+// the lowest free slot; if it is BLOCKED one more pass takes the update back and finds how long
+// the head must stay blocked (below).
 //
 // Arithmetic is 32 bit, wrapping: every TRUE value that is compared lies in [-M, 2M] and the
 // host takes this kernel only when M < 2^30, so the wrapped result read as int32 is exact.
@@ -47,8 +50,8 @@
 //    outputs are written.
 //  * otherwise the two-level shared-memory bitmap of svf_state.cuh and (s, o, id, a) records in
 //    priority order in global memory.
-// The two lowest waiting ranks are cached in registers (`head`, `second`; second's record is
-// fetched one admission ahead).  ARRIVALS come from a 32-wide register window over
+// The head of the queue is cached in registers (non-QREG: also the second, whose record is
+// fetched one admission ahead to hide the L2 latency).  ARRIVALS come from a 32-wide register window over
 // (a, s, o, rank), refilled once per 32 arrivals.  OUTPUTS (start, finish, latency word) are
 // buffered one admission per lane and written 32 at a time; p99 (nearest rank) is a radix selection
 // over the instance's latencies by the same thread group at the end of the instance.
