@@ -406,6 +406,42 @@ int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t 
                                  peak_kv, rounds, decisions, status);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT-2: the volume lower bound of Proposition 3.1 (Eq. 5) for burst input,
+ *     M * TEL(OPT) >= LB = sum_{j=1..N} sum_{i=1..j} vol_(i),   vol_(1) <= ... <= vol_(N),
+ * written as printed: sort the volumes (Eq. 1), then for every j add the sum of the first j.
+ * lb_out[j] = LB of instance j (int64); status_out[j] = ST_EOVERFLOW if LB >= 2^63 (lb 0),
+ * ST_ERANGE if some o < 1 or s < 0.  Arrivals are not looked at: the bound is about the burst
+ * version of the instance.
+ * ---------------------------------------------------------------------------------------- */
+int svf_ref_volume_lower_bound(int64_t n_instances, const int64_t *offsets, const int32_t *prompt,
+                               const int32_t *output, int64_t *lb_out, int32_t *status_out)
+{
+    if (n_instances < 0) return ST_EINVAL;
+    for (int64_t j = 0; j < n_instances; ++j) {
+        int64_t lo = offsets[j], n = offsets[j + 1] - offsets[j];
+        int32_t st = ST_OK;
+        int64_t *vol = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
+        for (int64_t i = 0; i < n; ++i) {
+            if (output[lo + i] < 1 || prompt[lo + i] < 0) st = ST_ERANGE;
+            vol[i] = ref_key(POL_SVF, prompt[lo + i], output[lo + i], 0, 0, 0, 0);
+        }
+        unsigned __int128 lb = 0, prefix = 0;
+        if (st == ST_OK) {
+            qsort(vol, (size_t)n, sizeof(int64_t), cmp_i64);
+            for (int64_t jj = 0; jj < n; ++jj) {      /* inner sum of Eq. 5 carried along */
+                prefix += (unsigned __int128)vol[jj];
+                lb += prefix;
+            }
+            if (lb >> 63) { st = ST_EOVERFLOW; lb = 0; }
+        }
+        free(vol);
+        lb_out[j] = (int64_t)lb;
+        if (status_out) status_out[j] = st;
+    }
+    return ST_OK;
+}
+
 int svf_ref_max_threads(void)
 {
 #ifdef _OPENMP

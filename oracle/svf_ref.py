@@ -149,3 +149,18 @@ def bruteforce_opt(s, o, M):
     if rc != OK:
         raise RuntimeError(f"svf_ref_bruteforce_opt failed: {rc}")
     return int(opt.value), start, int(nodes.value)
+
+
+def volume_lower_bound(trace):
+    """Prop. 3.1 (Eq. 5): LB_j = sum_j sum_{i<=j} vol_(i) per instance, so that for burst input
+    M * TEL(any schedule) >= LB.  Returns (lb[int64 I], status[int32 I])."""
+    I = trace.n_instances
+    off = np.ascontiguousarray(trace.offsets, dtype=np.int64)
+    s, o = _i32(trace.prompt), _i32(trace.output)
+    lb = np.zeros(I, np.int64)
+    st = np.zeros(I, np.int32)
+    rc = lib().svf_ref_volume_lower_bound(C.c_int64(I), _p(off, C.c_int64), _p(s, C.c_int32), _p(o, C.c_int32),
+                                          _p(lb, C.c_int64), _p(st, C.c_int32))
+    if rc != OK:
+        raise RuntimeError(f"svf_ref_volume_lower_bound failed: {rc}")
+    return lb, st

@@ -128,3 +128,54 @@ def test_config2_oracle_against_validator(oracle):
         tel[policy] = info["total_latency"]
         assert info["blocked_checked"] > 0
     assert tel[0] >= int(tr.output.astype(np.int64).sum())
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-2: the volume lower bound of Prop. 3.1 as an output of its own
+# ---------------------------------------------------------------------------------------------
+def _burst(tr):
+    tr.arrival[:] = 0
+    return tr
+
+
+def test_volume_lower_bound_closed_forms(oracle):
+    """Eq. 5 against the weighted form Eq. 12: sum_i (N - i + 1) vol_(i), computed
+    here in Python integers from the staircase definition of the volume (Eq. 3c), and against a
+    value worked out by hand."""
+    # by hand: (s, o) = (2,3), (1,2), (3,1): volumes 12, 5, 4 -> sorted 4, 5, 12 -> 4 + 9 + 21 = 34
+    tr = T._one("exA", np.zeros(3, np.int32), np.array([2, 1, 3]), np.array([3, 2, 1]), np.zeros(3, np.uint8), 8, 1, 1)
+    lb, st = oracle.volume_lower_bound(tr)
+    assert int(lb[0]) == 34 and int(st[0]) == 0
+    parts = [T.random_small(900 + i, 1 + 7 * i, 40, 30, 10 ** 6) for i in range(12)]
+    tr = T.concat(parts, "lb", 10 ** 6, 2, 8)
+    lb, st = oracle.volume_lower_bound(tr)
+    for j, p_ in enumerate(parts):
+        vol = sorted(sum(int(s) + k for k in range(1, int(o) + 1)) for s, o in zip(p_.prompt, p_.output))
+        n = len(vol)
+        assert int(lb[j]) == sum((n - i) * v for i, v in enumerate(vol)) and int(st[j]) == 0
+    # identical requests: LB = vol * N (N + 1) / 2; empty instance: 0
+    tr = T._one("same", np.zeros(50, np.int32), np.full(50, 7), np.full(50, 4), np.zeros(50, np.uint8), 100, 1, 1)
+    assert int(oracle.volume_lower_bound(tr)[0][0]) == (7 * 4 + 10) * 50 * 51 // 2
+    bad = T.random_small(3, 5, 9, 9, 50)
+    bad.output[2] = 0
+    assert int(oracle.volume_lower_bound(bad)[1][0]) == oracle.ERANGE
+
+
+def test_volume_lower_bound_bounds_every_schedule_and_the_optimum(oracle):
+    """M * TEL >= LB for the brute-force optimum and for all four policies on burst input
+    (Prop. 3.1); and the SVF certificate of Thm 3.2's proof (Lemma G.2 summed over requests,
+    P:L503-505): (TEL(SVF) - sum o) (M - p_max) <= 2 LB."""
+    for seed in range(40):
+        tr = T.config1(seed)
+        lb = int(oracle.volume_lower_bound(tr)[0][0])
+        opt, _, _ = oracle.bruteforce_opt(tr.prompt, tr.output, tr.M)
+        assert tr.M * opt >= lb
+        for policy in range(4):
+            assert tr.M * int(oracle.simulate(tr, policy).total_latency[0]) >= lb
+    for seed in range(10):
+        tr = _burst(T.config3(n_instances=1, n=400, lam=4.0, M=60_000, first_instance=seed))
+        lb = int(oracle.volume_lower_bound(tr)[0][0])
+        tel = int(oracle.simulate(tr, oracle.SVF).total_latency[0])
+        pmax = int((tr.prompt.astype(np.int64) + tr.output).max())
+        assert tr.M * tel >= lb
+        assert (tel - tr.request_steps) * (tr.M - pmax) <= 2 * lb
