@@ -355,6 +355,7 @@ def run_ours(args):
     if not args.no_extras:
         line["kernels"] = kernel_extras(B, torch, dev, peak)
         line["configs"] = config_extras(B, torch, dev)
+        line["ratio_to_lower_bound"] = bound_extras(B, torch, dev, args)
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args)
     print(json.dumps(line), flush=True)
@@ -428,6 +429,26 @@ def config_extras(B, torch, dev):
                         "request_steps_per_sec": tr.request_steps / ms * 1e3,
                         "decisions_per_sec": int(out.decisions.sum().item()) / ms * 1e3,
                         "total_latency": int(out.total_latency.sum().item())})
+    return res
+
+
+def bound_extras(B, torch, dev, args):
+    """the burst version of the bench batch (all arrivals at 0): TEL(policy) * M
+    over the volume lower bound of Prop. 3.1 -- an upper bound on each policy's approximation
+    ratio where the optimum cannot be computed (Thm 3.2 bounds SVF's true ratio by 1 + 2/(1-alpha))."""
+    tr = T.config3(n_instances=min(args.instances, 4096), n=args.requests, lam=args.lam)
+    tr.arrival[:] = 0
+    d = B.DeviceTrace.from_host(tr, device=dev)
+    ms = _time_cuda(torch, lambda: B.svf_volume_lower_bound(d), reps=3)
+    lb, st = B.svf_volume_lower_bound(d)
+    outs = B.svf_simulate_policies(d, POLICIES, want=("total_latency", "status"))
+    torch.cuda.synchronize()
+    lbf = lb.double()
+    res = {"workload": f"burst version of the bench batch ({tr.n_instances} x {args.requests}, all arrivals at t=0)",
+           "lower_bound_ms": ms, "lower_bound_status_ok": bool(int(st.abs().sum().item()) == 0)}
+    for name, out in zip(POLICY_NAMES, outs):
+        r = out.total_latency.double() * float(tr.M) / lbf
+        res[name] = {"mean": float(r.mean().item()), "max": float(r.max().item())}
     return res
 
 

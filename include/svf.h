@@ -142,6 +142,19 @@ size_t svf_simulate_policies_workspace_bytes(const svf_trace_t* trace, int n_pol
 int svf_simulate_policies(const svf_trace_t* trace, int n_policies, const int* policies, int64_t M,
                           const svf_result_t* outs, void* ws, size_t ws_bytes, void* stream);
 
+/* the volume lower bound of Proposition 3.1 (Eq. 5).  With the
+ * volumes of an instance sorted ascending, vol_(1) <= ... <= vol_(n) (Eq. 1),
+ *     lb_out[j] = sum_{k=1..n} sum_{i=1..k} vol_(i) = sum_i (n - i + 1) vol_(i),
+ * so that for BURST input (all requests present at the start) M * TEL(any feasible schedule) >=
+ * lb_out[j]; TEL(policy) * M / lb_out[j] upper-bounds the policy's approximation ratio where the
+ * optimum cannot be computed.  Arrivals, `bit` and `output_key` are not read.  lb_out: [dev] [I]
+ * int64; status_out: [dev] [I] int32 or NULL: SVF_OK, SVF_ERANGE (o_i < 1 or s_i < 0),
+ * SVF_EOVERFLOW (bound >= 2^63), SVF_EINVAL (bad offsets); lb_out[j] = 0 unless SVF_OK.
+ * Keys + the same presort as svf_simulate + one reduction kernel. */
+size_t svf_volume_lower_bound_workspace_bytes(const svf_trace_t* trace);
+int svf_volume_lower_bound(const svf_trace_t* trace, int64_t* lb_out, int32_t* status_out, void* ws,
+                           size_t ws_bytes, void* stream);
+
 /* The sort subsystem on its own (a3), for tests and measurement: ascending, stable LSD
  * onesweep radix sort of n 64-bit words on the bit range [bit_lo, bit_hi) (0 <= bit_lo <
  * bit_hi <= 64; words that agree on that range keep their input order).  words_in: [dev][n]

@@ -23,7 +23,7 @@ ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
 EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_workspace_bytes",
            "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies",
-           "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
+           "svf_volume_lower_bound_workspace_bytes", "svf_volume_lower_bound", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
            "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
            "svf_simulate_work_counts")
 
@@ -78,6 +78,11 @@ def lib():
         L.svf_simulate_policies.restype = C.c_int
         L.svf_simulate_policies.argtypes = [C.POINTER(_Trace), C.c_int, C.POINTER(C.c_int), C.c_int64,
                                             C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.svf_volume_lower_bound_workspace_bytes.restype = C.c_size_t
+        L.svf_volume_lower_bound_workspace_bytes.argtypes = [C.POINTER(_Trace)]
+        L.svf_volume_lower_bound.restype = C.c_int
+        L.svf_volume_lower_bound.argtypes = [C.POINTER(_Trace), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
+                                             C.c_void_p]
         L.svf_sort_workspace_bytes.restype = C.c_size_t
         L.svf_sort_workspace_bytes.argtypes = [C.c_int64, C.c_int, C.c_int]
         L.svf_sort_words.restype = C.c_int
@@ -363,3 +368,20 @@ def svf_simulate_policies(dt: DeviceTrace, policies, M: Optional[int] = None, ou
     for o in outs:
         o._ws = ws
     return outs
+
+
+def svf_volume_lower_bound(dt: DeviceTrace, ws: Optional[torch.Tensor] = None, stream=None):
+    """Prop. 3.1 lower bound per instance (int64 [I]) and its status (int32 [I])."""
+    if not dt.offsets.is_cuda:
+        raise TypeError("svf_volume_lower_bound needs device tensors (the library has no CPU path)")
+    dev = dt.offsets.device
+    tr = dt.c_struct()
+    need = int(lib().svf_volume_lower_bound_workspace_bytes(C.byref(tr)))
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    lb = torch.zeros(max(dt.n_instances, 1), dtype=torch.int64, device=dev)
+    st = torch.zeros(max(dt.n_instances, 1), dtype=torch.int32, device=dev)
+    rc = lib().svf_volume_lower_bound(C.byref(tr), C.c_void_p(lb.data_ptr()), C.c_void_p(st.data_ptr()),
+                                      C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
+    _check(rc, "svf_volume_lower_bound")
+    return lb[: dt.n_instances], st[: dt.n_instances]

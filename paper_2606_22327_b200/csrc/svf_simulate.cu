@@ -279,6 +279,53 @@ __global__ void k_sim_p99(int64_t I, const int64_t* __restrict__ off, const Sort
     p99[j] = v;
 }
 
+// ---- NEXT-2: the volume lower bound of Proposition 3.1 (Eq. 5) -------------------------
+// LB_j = sum_{r=0..n-1} (n - r) vol_(r), volumes ascending = the SVF priority order of the
+// presort; one CTA per instance, 128-bit accumulation, overflow (>= 2^63) reported, never wrapped.
+__global__ void __launch_bounds__(256) k_volume_lb(int64_t I, int64_t N, int64_t max_instance,
+                                                   const int64_t* __restrict__ off, const int32_t* __restrict__ s,
+                                                   const int32_t* __restrict__ o, const uint32_t* __restrict__ order,
+                                                   int64_t* __restrict__ lb_out, int32_t* __restrict__ status_out)
+{
+    __shared__ unsigned long long part[8][2];
+    __shared__ uint32_t flags_s;
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    for (int64_t j = blockIdx.x; j < I; j += gridDim.x) {
+        const int64_t base = off[j], n = off[j + 1] - base;
+        uint32_t flags = 0;
+        if (n < 0 || n > max_instance || base < 0 || base + (n > 0 ? n : 0) > N || off[0] != 0 || off[I] != N) flags |= F_LAYOUT;
+        if (tid == 0) flags_s = 0;
+        __syncthreads();
+        unsigned __int128 acc = 0;
+        if (!flags) {
+            for (int64_t r = tid; r < n; r += 256) {
+                const int64_t i = base + order[base + r];
+                const int32_t si = s[i], oi = o[i];
+                if (oi < 1 || si < 0) flags |= F_RANGE;
+                acc += (unsigned __int128)priority_key(SVF_SVF, si, oi, 0, 0u, 0, 0) * (unsigned long long)(n - r);
+            }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            const unsigned long long lo = __shfl_xor_sync(FULL, (unsigned long long)acc, d);
+            const unsigned long long hi = __shfl_xor_sync(FULL, (unsigned long long)(acc >> 64), d);
+            acc += ((unsigned __int128)hi << 64) | lo;
+        }
+        flags = __reduce_or_sync(FULL, flags);
+        if (lane == 0) { part[wrp][0] = (unsigned long long)acc; part[wrp][1] = (unsigned long long)(acc >> 64); if (flags) atomicOr(&flags_s, flags); }
+        __syncthreads();
+        if (tid == 0) {
+            unsigned __int128 tot = 0;
+            for (int w = 0; w < 8; ++w) tot += ((unsigned __int128)part[w][1] << 64) | part[w][0];
+            uint32_t f = flags_s;
+            if (!f && (tot >> 63)) f |= F_OVERFLOW;
+            lb_out[j] = f ? 0 : (int64_t)tot;
+            if (status_out) status_out[j] = status_from_flags(f);
+        }
+        __syncthreads();
+    }
+}
+
 struct SimWs {
     SortWs sort;            // sized for the larger of the two sorts
     uint64_t* words0;       // [N] sort ping-pong (device-wide presort, p99 sort of the wide kernel)
@@ -690,6 +737,57 @@ extern "C" int svf_simulate_policies(const svf_trace_t* tr, int n_policies, cons
 {
     g_launches_sim = 0;
     return simulate_impl(tr, n_policies, policies, M, outs, ws, ws_bytes, stream);
+}
+
+extern "C" size_t svf_volume_lower_bound_workspace_bytes(const svf_trace_t* tr) { return sim_workspace_bytes(tr, 1); }
+
+extern "C" int svf_volume_lower_bound(const svf_trace_t* tr, int64_t* lb_out, int32_t* status_out, void* ws,
+                                      size_t ws_bytes, void* stream)
+{
+    g_launches_sim = 0;
+    if (!tr || !lb_out) return SVF_EINVAL;
+    const int64_t I = tr->n_instances, N = tr->n_requests;
+    if (I < 0 || N < 0 || N >= ((int64_t)1 << 30) || tr->max_instance < 0 || tr->max_instance > N) return SVF_EINVAL;
+    if (I == 0) return SVF_OK;
+    if (!tr->offsets || (N > 0 && (!tr->prompt || !tr->output))) return SVF_EINVAL;
+    SimConfig c = sim_config(tr, 0, 1);
+    if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;
+    if (!ws) return SVF_EWORKSPACE;
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
+    SimWs w;
+    sim_ws_layout(&w, base, tr, c, 0, 1);
+    if (w.total - w.slot_bytes * (size_t)w.grid_slots > avail) return SVF_EWORKSPACE;
+    // volumes ascending = the SVF order under the TRUE lengths (no predicted keys here)
+    if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
+        if (seg_sort_keys(SVF_SVF, I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, nullptr,
+                          tr->prompt /* a is not read by the SVF key */, nullptr, 0, 0, w.order[0], w.rank[0], nullptr, st,
+                          &g_launches_sim))
+            return SVF_ECUDA;
+    } else if (N > 0) {
+        SimArgs g;
+        g.I = I; g.N = N; g.M = 0; g.max_instance = tr->max_instance;
+        g.policy = SVF_SVF; g.O0 = 0; g.O1 = 0; g.sb = c.sb;
+        g.off = tr->offsets; g.a = tr->prompt; g.s = tr->prompt; g.o = tr->output; g.okey = nullptr; g.bit = nullptr;
+        g.req = nullptr;
+        int64_t blocks = ceil_div(N, 256);
+        const int64_t capb = (int64_t)sm_count() * 8;
+        if (blocks > capb) blocks = capb;
+        k_sim_pack<<<(unsigned)blocks, 256, 0, st>>>(g, w.words0);
+        ++g_launches_sim;
+        if (sort_u64(w.sort, w.words0, w.words1, w.words0, N, c.sort_lo, c.sort_hi, st, &g_launches_sim)) return SVF_ECUDA;
+        k_sim_rank<<<(unsigned)blocks, 256, 0, st>>>(g, w.sort.plan, w.order[0], w.rank[0]);
+        ++g_launches_sim;
+    }
+    int64_t grid = (int64_t)sm_count() * 8;
+    if (grid > I) grid = I;
+    k_volume_lb<<<(unsigned)grid, 256, 0, st>>>(I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, w.order[0],
+                                                lb_out, status_out);
+    ++g_launches_sim;
+    return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
 }
 
 extern "C" void svf_set_profiling(int mode) { g_profiling = mode == 2 ? 2 : (mode ? 1 : 0); if (mode != 2) g_counts_dev = nullptr; }

@@ -399,3 +399,50 @@ def test_admit_agrees_with_simulator_states(B, oracle):
               (s[run] + t - k[run]).astype(np.int32), (k[run] + o[run] - t).astype(np.int32))
         n_adm = _admit_both(B, oracle, 0, tr.M, st)
         assert n_adm == int((k[wait] == t).sum())
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-2: the volume lower bound of Prop. 3.1
+# ---------------------------------------------------------------------------------------------
+def test_volume_lower_bound_matches_oracle(B, oracle):
+    import torch
+    parts = [T.random_small(700 + i, (i * 37) % 300, 60, 50, 10 ** 6) for i in range(40)]
+    parts[7].output[3] = 0                                   # ERANGE
+    cases = [T.concat(parts, "lb-ragged", 10 ** 6, 2, 8), T.config3(n_instances=50, n=1000, lam=4.0),
+             T.config4(n=30_000), T.config5(n_instances=3)]
+    for tr in cases:
+        lb, st = B.svf_volume_lower_bound(B.DeviceTrace.from_host(tr))
+        torch.cuda.synchronize()
+        rlb, rst = oracle.volume_lower_bound(tr)
+        assert np.array_equal(lb.cpu().numpy(), rlb), tr.name
+        assert np.array_equal(st.cpu().numpy(), rst), tr.name
+    # overflow is reported, not wrapped: 100,000 requests of volume 2.25e9 each -> 1.1e19 >= 2^63
+    n = 100_000
+    big = T._one("big", np.zeros(n, np.int32), np.full(n, 60_000), np.full(n, 30_000), np.zeros(n, np.uint8), 10 ** 9, 1, 1)
+    lb, st = B.svf_volume_lower_bound(B.DeviceTrace.from_host(big))
+    rlb, rst = oracle.volume_lower_bound(big)
+    assert int(st[0]) == oracle.EOVERFLOW == int(rst[0]) and int(lb[0]) == 0 == int(rlb[0])
+
+
+def test_ratio_to_lower_bound_at_scale(B, oracle):
+    """Burst version of configs[2] at full size: M * TEL >= LB for every policy and instance
+    (Prop. 3.1), and the SVF certificate of Thm 3.2's proof (TEL - sum o)(M - p_max) <= 2 LB
+    (Lemma G.2 summed) -- properties that hold at any size, on GPU outputs only."""
+    import torch
+    tr = T.config3(n_instances=4096, lam=4.0)
+    tr.arrival[:] = 0
+    dt = B.DeviceTrace.from_host(tr)
+    lb, st = B.svf_volume_lower_bound(dt)
+    outs = B.svf_simulate_policies(dt, [0, 1, 2, 3], want=("total_latency", "status"))
+    torch.cuda.synchronize()
+    lb = lb.cpu().numpy()
+    assert not st.cpu().numpy().any()
+    sum_o = np.add.reduceat(tr.output.astype(np.int64), tr.offsets[:-1])
+    pmax = np.maximum.reduceat(tr.prompt.astype(np.int64) + tr.output, tr.offsets[:-1])
+    for pol, out in enumerate(outs):
+        tel = out.total_latency.cpu().numpy()
+        assert (tr.M * tel >= lb).all(), pol
+    tel_svf = outs[0].total_latency.cpu().numpy()
+    assert ((tel_svf - sum_o) * (tr.M - pmax) <= 2 * lb).all()
+    sub = np.arange(0, 4096, 128)
+    assert np.array_equal(lb[sub], oracle.volume_lower_bound(tr.subset(sub))[0])
