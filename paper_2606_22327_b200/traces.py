@@ -291,3 +291,36 @@ def with_predicted_lengths(trace: Trace, sigma: float = 0.5, seed: int = 0, hi: 
     return Trace(trace.name + f"[pred sigma={sigma:g}]", trace.offsets.copy(), trace.arrival.copy(),
                  trace.prompt.copy(), trace.output.copy(), trace.bit.copy(), trace.M, trace.O0, trace.O1,
                  dict(trace.meta), ok)
+
+
+# ---------------------------------------------------------------------------------------------
+# Stochastic-regime workload: the paper's reference model of App. H
+# (PAPER.md:866-870): Poisson arrivals, o ~ Geo(mu) truncated at the generation budget
+# ---------------------------------------------------------------------------------------------
+def geometric_int(seed: int, stream: int, n: int, mu: float, hi: int) -> np.ndarray:
+    """o = min(hi, 1 + floor(ln(1-u) / ln(1-mu))): Pr(o = k) = mu (1-mu)^(k-1) on {1, 2, ..}
+    (inverse CDF), truncated at ``hi`` (the paper's "maximum generation budget")."""
+    u = uniform(seed, stream, n)
+    k = 1 + np.floor(np.log1p(-u) / math.log1p(-mu))
+    return np.clip(k, 1, hi).astype(np.int32)
+
+
+def stochastic(n_instances: int = 64, n: int = 1000, lam: float = 1.0, mean_o: float = 293.0,
+               o_hi: int = 4096, M: int = 300_000, first_instance: int = 0) -> Trace:
+    """Poisson(lam) arrivals, o ~ Geo(1/mean_o) truncated at o_hi (mean 293 and budget 4,096 are the
+    paper's calibration, PAPER.md:870), prompts as config 2.  1-bit constants follow Thm 3.5's
+    conditional-expectation recipe at theta = mean_o, rounded to integers:
+    O0 = 1/mu - theta q^theta / (1 - q^theta), O1 = theta + 1/mu, q = 1 - mu."""
+    mu = 1.0 / mean_o
+    theta = int(round(mean_o))
+    q_t = (1.0 - mu) ** theta
+    O0 = max(1, int(round(1.0 / mu - theta * q_t / (1.0 - q_t))))
+    O1 = max(1, int(round(theta + 1.0 / mu)))
+    parts = []
+    for j in range(first_instance, first_instance + n_instances):
+        sd = instance_seed(6, j, variant=int(round(lam * 16)))
+        a = poisson_arrivals(sd, n, lam)
+        s = lognormal_int(sd, _ST_S1, _ST_S2, n, 600.0, 0.8, 16, 4096)
+        o = geometric_int(sd, _ST_O1, n, mu, o_hi)
+        parts.append(_one("", a, s, o, (o > theta).astype(np.uint8), M, O0, O1))
+    return concat(parts, f"geo[lam={lam:g},1/mu={mean_o:g}]", M, O0, O1, {"config": 6, "lam": lam, "mu": mu})

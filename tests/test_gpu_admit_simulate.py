@@ -446,3 +446,11 @@ def test_ratio_to_lower_bound_at_scale(B, oracle):
     assert ((tel_svf - sum_o) * (tr.M - pmax) <= 2 * lb).all()
     sub = np.arange(0, 4096, 128)
     assert np.array_equal(lb[sub], oracle.volume_lower_bound(tr.subset(sub))[0])
+
+
+def test_stochastic_reference_workload(B, oracle):
+    """NEXT-3: Poisson arrivals, geometric outputs (App. H reference model), light and heavy load."""
+    for lam, M in ((0.05, 300_000), (1.0, 300_000), (2.0, 120_000)):
+        tr = T.stochastic(n_instances=48, n=600, lam=lam, M=M)
+        for policy in range(4):
+            check(B, oracle, tr, policy, ctx=f"{tr.name} M={M} policy {policy}")

@@ -322,3 +322,41 @@ def test_predicted_keys_schedules_pass_the_validator(oracle, policy):
     bad = T.with_predicted_lengths(T.random_small(1, 10, 9, 11, 26), sigma=0.5)
     bad.output_key[3] = 0
     assert int(oracle.simulate(bad, policy).status[0]) == oracle.ERANGE
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: the stochastic reference workload of App. H -- generator facts the paper
+# prints, and the oracle on it
+# ---------------------------------------------------------------------------------------------
+def test_geometric_reference_model_constants():
+    """PAPER.md:870: 1/mu = 293 and a 4,096-token budget give Pr(o > 4096) ~ 8.29e-7;
+    PAPER.md:953 (Eq. 101): E[o] = 1/mu, E[o^2] = (2-mu)/mu^2, E[vol] = E[s]/mu + 1/mu^2."""
+    mu = 1.0 / 293.0
+    assert abs((1.0 - mu) ** 4096 - 8.29e-7) < 0.005e-7
+    o = T.geometric_int(T.instance_seed(6, 0), 4, 2_000_000, mu, 1 << 30).astype(np.float64)
+    assert abs(o.mean() * mu - 1.0) < 0.005
+    assert abs((o * o).mean() * mu * mu / (2.0 - mu) - 1.0) < 0.01
+    assert o.min() == 1
+    # the share of draws above the budget matches the geometric tail (1-mu)^k at a visible k
+    assert abs((o > 1000).mean() / (1.0 - mu) ** 1000 - 1.0) < 0.03
+    tr = T.stochastic(n_instances=200, n=1000, lam=1.0)
+    vol = tr.prompt.astype(np.float64) * tr.output + (tr.output.astype(np.float64) ** 2 + tr.output) / 2
+    assert abs(vol.mean() / (tr.prompt.mean() / mu + 1.0 / mu ** 2) - 1.0) < 0.03
+    assert tr.O0 == 123 and tr.O1 == 586           # Thm 3.5 recipe at theta = 293 (PAPER.md:191)
+
+
+def test_oracle_on_the_stochastic_workload(oracle):
+    """Under light load (rho << 1) nobody waits: TEL = sum o; the validator accepts the schedules
+    under load; more load never helps (same requests, denser arrivals cannot lower SVF's TEL below
+    sum o)."""
+    from oracle import validator
+    light = T.stochastic(n_instances=3, n=300, lam=0.05, M=300_000)
+    r = oracle.simulate(light, oracle.SVF)
+    assert int(r.total_latency.sum()) == light.request_steps
+    heavy = T.stochastic(n_instances=2, n=300, lam=2.0, M=60_000)
+    for policy in range(4):
+        rr = oracle.simulate(heavy, policy)
+        assert (rr.total_latency >= np.add.reduceat(heavy.output.astype(np.int64), heavy.offsets[:-1])).all()
+        one = heavy.instance(0)
+        r1 = oracle.simulate(one, policy)
+        validator.validate(one, policy, r1.start, finish=r1.finish)
