@@ -454,3 +454,25 @@ def test_stochastic_reference_workload(B, oracle):
         tr = T.stochastic(n_instances=48, n=600, lam=lam, M=M)
         for policy in range(4):
             check(B, oracle, tr, policy, ctx=f"{tr.name} M={M} policy {policy}")
+
+
+def test_more_running_requests_than_register_slots(B, oracle):
+    """Running sets far beyond the register slots of a group (512 per warp, 2048 / 4096 per CTA):
+    the ext slots (global memory under the warp kernel, shared / global under the CTA kernels) hold
+    the overflow.  Long outputs, small prompts, a budget that fits almost everything at once."""
+    def crowd(I, n, seed):
+        parts = []
+        for j in range(I):
+            sd = T.instance_seed(88, seed * 1000 + j)
+            a = np.sort(T.uniform_int(sd, 1, n, 0, 40))
+            s = T.uniform_int(sd, 2, n, 0, 6)
+            o = T.uniform_int(sd, 3, n, 150, 400)
+            parts.append(T._one("", a, s, o, (o > 250).astype(np.uint8), 0, 200, 300))
+        return parts
+    for I, n, M in ((40, 1000, 330_000), (600, 900, 200_000), (3, 5000, 1_500_000), (1, 9000, 2_500_000)):
+        tr = T.concat(crowd(I, n, n), f"crowd{I}x{n}", M, 200, 300)
+        for policy in (0, 1, 3):
+            ref, got = check(B, oracle, tr, policy, ctx=f"{tr.name} policy {policy}")
+        # the point of the case: most of an instance runs at once
+        started_early = (ref.start[: tr.offsets[1]] < 150).sum()
+        assert started_early > 0.6 * n
