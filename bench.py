@@ -464,7 +464,7 @@ def cpu_baseline(args):
     while True:
         oracle_step(svf_ref, sample, threads)
         reps += 1
-        if time.perf_counter() - t0 > 10.0 or reps >= 8:
+        if time.perf_counter() - t0 > 12.0 or reps >= 40:
             break
     dt = time.perf_counter() - t0
     return {"value": sample.request_steps * len(POLICIES) * reps / dt, "unit": UNIT, "cores": threads,
