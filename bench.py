@@ -356,6 +356,12 @@ def run_ours(args):
         line["kernels"] = kernel_extras(B, torch, dev, peak)
         line["configs"] = config_extras(B, torch, dev)
         line["ratio_to_lower_bound"] = bound_extras(B, torch, dev, args)
+        # the paper's own metrics on the bench batch, per policy, this rank
+        from paper_2606_22327_b200 import report as RP
+        line["paper_metrics"] = {
+            name: RP.paper_metrics(dt_dev.arrival, dt_dev.output, o.finish[: batch.n_requests], dt_dev.offsets, o.status)
+            for name, o in zip(POLICY_NAMES, outs)}
+        line["paper_metrics"]["units"] = "per-token latency in model steps per output token; throughput in tokens per step per instance"
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args)
     print(json.dumps(line), flush=True)
