@@ -32,22 +32,36 @@ __global__ void __launch_bounds__(256) k_keys(int64_t n, const int32_t* __restri
     const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (VEC) {
         const int64_t n4 = n >> 2;
-        for (int64_t q = gid; q < n4; q += stride) {
-            int4 vs = make_int4(0, 0, 0, 0), vo = make_int4(0, 0, 0, 0), va = make_int4(0, 0, 0, 0);
-            uint32_t vb = 0;
-            if (POLICY == SVF_SVF || POLICY == SVF_SVF_1BIT) vs = ld_stream(reinterpret_cast<const int4*>(s) + q);
-            if (POLICY == SVF_SVF || POLICY == SVF_SJF) vo = ld_stream(reinterpret_cast<const int4*>(o) + q);
-            if (POLICY == SVF_FCFS) va = ld_stream(reinterpret_cast<const int4*>(a) + q);
-            if (POLICY == SVF_SVF_1BIT) vb = __ldg(reinterpret_cast<const uint32_t*>(bit) + q);
-            const uint64_t i0 = (uint64_t)q << 2;
-            uint64_t k0 = priority_key(POLICY, vs.x, vo.x, va.x, vb & 0xffu, O0, O1);
-            uint64_t k1 = priority_key(POLICY, vs.y, vo.y, va.y, (vb >> 8) & 0xffu, O0, O1);
-            uint64_t k2 = priority_key(POLICY, vs.z, vo.z, va.z, (vb >> 16) & 0xffu, O0, O1);
-            uint64_t k3 = priority_key(POLICY, vs.w, vo.w, va.w, (vb >> 24) & 0xffu, O0, O1);
-            overflow |= ((k0 | k1 | k2 | k3) >> 32) != 0;
-            ulonglong2* out = reinterpret_cast<ulonglong2*>(words + i0);
-            st_stream(out, (k0 << 32) + i0, (k1 << 32) + (i0 + 1));
-            st_stream(out + 1, (k2 << 32) + (i0 + 2), (k3 << 32) + (i0 + 3));
+        // two groups of four requests per thread and iteration: eight independent 128-bit loads in
+        // flight before the first store
+        for (int64_t q0 = gid; q0 < n4; q0 += 2 * stride) {
+            int4 vs[2], vo[2], va[2];
+            uint32_t vb[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int64_t q = q0 + u * stride;
+                vs[u] = vo[u] = va[u] = make_int4(0, 0, 0, 0); vb[u] = 0;
+                if (q < n4) {
+                    if (POLICY == SVF_SVF || POLICY == SVF_SVF_1BIT) vs[u] = ld_stream(reinterpret_cast<const int4*>(s) + q);
+                    if (POLICY == SVF_SVF || POLICY == SVF_SJF) vo[u] = ld_stream(reinterpret_cast<const int4*>(o) + q);
+                    if (POLICY == SVF_FCFS) va[u] = ld_stream(reinterpret_cast<const int4*>(a) + q);
+                    if (POLICY == SVF_SVF_1BIT) vb[u] = __ldg(reinterpret_cast<const uint32_t*>(bit) + q);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int64_t q = q0 + u * stride;
+                if (q >= n4) break;
+                const uint64_t i0 = (uint64_t)q << 2;
+                uint64_t k0 = priority_key(POLICY, vs[u].x, vo[u].x, va[u].x, vb[u] & 0xffu, O0, O1);
+                uint64_t k1 = priority_key(POLICY, vs[u].y, vo[u].y, va[u].y, (vb[u] >> 8) & 0xffu, O0, O1);
+                uint64_t k2 = priority_key(POLICY, vs[u].z, vo[u].z, va[u].z, (vb[u] >> 16) & 0xffu, O0, O1);
+                uint64_t k3 = priority_key(POLICY, vs[u].w, vo[u].w, va[u].w, (vb[u] >> 24) & 0xffu, O0, O1);
+                overflow |= ((k0 | k1 | k2 | k3) >> 32) != 0;
+                ulonglong2* out = reinterpret_cast<ulonglong2*>(words + i0);
+                st_stream(out, (k0 << 32) + i0, (k1 << 32) + (i0 + 1));
+                st_stream(out + 1, (k2 << 32) + (i0 + 2), (k3 << 32) + (i0 + 3));
+            }
         }
         // ragged tail (< 4 requests)
         const int64_t i = (n4 << 2) + gid;
