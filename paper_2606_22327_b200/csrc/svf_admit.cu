@@ -2,12 +2,15 @@
 // forward-looking check; P:L926 maxima at completion times).
 //   keys (svf_keys.cu) -> onesweep sort of the packed words on the key bits [32, 64)
 //   running set: words (2^32-1-rem, index) sorted the same way -> latest finish first
-//   k_admit: one CTA builds (f_j, A_j) with a block scan (svf_state.cuh), then pops the sorted
-//   queue while the check passes.
+//   k_admit: one CTA builds (f_j, A_j) in finish order with a block scan (svf_state.cuh) and checks
+//   the running set; then k_admit_slots (M < 2^30) takes the set into REGISTER SLOTS and pops the
+//   sorted queue with the fused evaluation pass of svf_sim_slots.cuh while the check passes;
+//   for M >= 2^30 k_admit itself pops the queue on the sorted (f, A) arrays in 64-bit.
 #include <limits.h>
 
 #include "svf_internal.cuh"
 #include "svf_state.cuh"
+#include "svf_sim_slots.cuh"
 
 namespace svf {
 
@@ -77,10 +80,12 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
                                                          int32_t* __restrict__ f, int64_t* __restrict__ A,
                                                          int64_t* __restrict__ n_admitted_out,
                                                          int32_t* __restrict__ admitted_idx_out,
-                                                         int32_t* __restrict__ status_out)
+                                                         int32_t* __restrict__ status_out,
+                                                         int* __restrict__ handoff /* NULL: admit here */)
 {
     __shared__ int scratch[2][64];
     __shared__ int64_t warp_tot[ADMIT_THREADS / 32];
+    if (handoff && threadIdx.x == 0) *handoff = 0;
     int parity = 0;
     const int tid = threadIdx.x;
 
@@ -114,6 +119,10 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
     __syncthreads();
     bad = Group<ADMIT_THREADS>::or_u32(bad, scratch, parity);
 
+    if (handoff && !bad) {       // the register-slot kernel takes over from the (f, A) arrays
+        if (tid == 0) *handoff = 1;
+        return;
+    }
     int64_t k = 0;
     if (!bad) {        // an infeasible running set admits nobody (every check would fail)
         const uint64_t* __restrict__ wsorted = wplan->result;
@@ -132,10 +141,106 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
     if (tid == 0) { *n_admitted_out = k; if (status_out) *status_out = SVF_OK; }
 }
 
+// a4 + a5 with the running set in REGISTER SLOTS (the passes of svf_sim_slots.cuh at t = 0): one
+// CTA, 16 slots per thread, the overflow in ext arrays; taken when M < 2^30.  Picks up the running
+// set (f, A) that k_admit built in finish order, then pops the sorted queue while the check holds.
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wait, const int32_t* __restrict__ w_s,
+                                                         const int32_t* __restrict__ w_o, int64_t n_run,
+                                                         const int32_t* __restrict__ r_kv,
+                                                         const SortPlan* __restrict__ wplan,
+                                                         const SortPlan* __restrict__ rplan,
+                                                         const int* __restrict__ handoff,
+                                                         const int32_t* __restrict__ f_arr, const int64_t* __restrict__ A_arr,
+                                                         int32_t* __restrict__ ef, uint32_t* __restrict__ eB,
+                                                         uint32_t* __restrict__ ec,
+                                                         int64_t* __restrict__ n_admitted_out,
+                                                         int32_t* __restrict__ admitted_idx_out,
+                                                         int32_t* __restrict__ status_out)
+{
+    constexpr int K = 16, WARPS = THREADS / 32, REGCAP = THREADS * K, TSHIFT = 8;
+    constexpr bool COUNT = false;
+    static_assert(THREADS == 256, "TSHIFT");
+    __shared__ int red[2][WARPS][3];
+    int rparity = 0;
+    long long cntE = 0, cntU = 0;
+    (void)cntE; (void)cntU;
+    if (*handoff == 0) return;               // data error or infeasible running set: k_admit has answered
+    const int tid = threadIdx.x;
+    const int Mi = (int)M;
+    const uint64_t* __restrict__ rsorted = rplan->result;
+    const uint64_t* __restrict__ wsorted = wplan->result;
+    const int R = (int)n_run;
+    int f[K]; uint32_t B[K], c[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const int q = k * THREADS + tid;
+        f[k] = 0; B[k] = 0; c[k] = 0;
+        if (q < R) { f[k] = f_arr[q]; B[k] = (uint32_t)A_arr[q] + (uint32_t)f[k]; c[k] = (uint32_t)r_kv[(uint32_t)rsorted[q]]; }
+    }
+    for (int q = REGCAP + tid; q < R; q += THREADS) {
+        const int e = q - REGCAP;
+        ef[e] = f_arr[q]; eB[e] = (uint32_t)A_arr[q] + (uint32_t)f_arr[q]; ec[e] = (uint32_t)r_kv[(uint32_t)rsorted[q]];
+    }
+    int hw = R;
+    const uint32_t t1 = 1u;                  // now = 0: a slot is live iff f > 0
+    int64_t k = 0;
+    uint32_t nh = 0; int32_t nsh = 0, noh = 0;
+    if (n_wait > 0) { nh = (uint32_t)wsorted[0]; nsh = w_s[nh]; noh = w_o[nh]; }
+    for (; k < n_wait; ++k) {
+        const uint32_t h = nh;
+        const int32_t sh = nsh, ohi = noh;
+        if (k + 1 < n_wait) { nh = (uint32_t)wsorted[k + 1]; nsh = w_s[nh]; noh = w_o[nh]; }   // one head ahead
+        if ((int64_t)sh + ohi > M) break;                    // could never run: blocked (and it blocks the rest)
+        const int fh = ohi;
+        const uint32_t oh = (uint32_t)ohi, fhu = (uint32_t)fh;
+        const uint32_t Kc = (uint32_t)sh - (uint32_t)Mi, add = (uint32_t)sh;
+        uint32_t acc = 0, dm = 0;
+        int viol = INT_MIN;
+        int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;
+        const int g4 = (kmax + 3) >> 2;
+        const bool use_ext = hw > REGCAP;
+        SVF_SLOT_GROUPS(g4, SVF_EVAL)
+        const uint32_t low = dm ? (dm & (0u - dm)) : (1u << (4 * g4));
+        int fkey = low < (1u << K) ? (int)((low << TSHIFT) | (uint32_t)tid) : INT_MAX;
+        int eidx = INT_MAX;
+        if (use_ext) {
+            for (int q = REGCAP + tid; q < hw; q += THREADS) {
+                const int e = q - REGCAP;
+                const int fk = ef[e];
+                const uint32_t x = (uint32_t)fk - t1;
+                if (fk >= fh) acc += ec[e] + fhu;
+                if (x < oh) { viol = __viaddmax_s32((int)eB[e], (int)Kc, viol); eB[e] += add + (uint32_t)fk; }
+                if (x >> 31) eidx = eidx < q ? eidx : q;
+            }
+        }
+        reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
+        const int Ah = sh + ohi + (int)acc;
+        if (viol > 0 || Ah > Mi) break;                      // blocked head: nobody may bypass it
+        const uint32_t Bh = (uint32_t)Ah + fhu;
+        int idx;
+        if (fkey != INT_MAX) {
+            const int ik = 31 - __clz(fkey >> TSHIFT);
+            const bool mine = (fkey & (THREADS - 1)) == tid;
+            idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
+            SVF_PUT16(ik, SVF_PUT)
+        } else {
+            if (use_ext) { uint32_t z = 0; int zmax = 0; reduce_add_max_min<THREADS>(z, zmax, eidx, red, rparity); }
+            idx = eidx == INT_MAX ? hw : eidx;
+            if (((idx - REGCAP) & (THREADS - 1)) == tid) { const int e = idx - REGCAP; ef[e] = fh; eB[e] = Bh; ec[e] = add; }
+        }
+        hw = idx + 1 > hw ? idx + 1 : hw;
+        if (tid == 0 && admitted_idx_out) admitted_idx_out[k] = (int32_t)h;
+    }
+    if (tid == 0) { *n_admitted_out = k; if (status_out) *status_out = SVF_OK; }
+}
+
 struct AdmitWs {
     SortWs wsort, rsort;
     uint64_t *w0, *w1, *r0, *r1;
     int32_t* f; int64_t* A;
+    int32_t* ef; uint32_t *eB, *ec;   // ext slots of the register-slot kernel
+    int* handoff;
     AdmitFlags* flags;
     size_t total;
 };
@@ -155,6 +260,10 @@ void admit_ws_layout(AdmitWs* w, char* base, int64_t n_wait, int64_t n_run)
     const size_t cap = (size_t)(n_wait + n_run + 1);
     w->A = (int64_t*)(base + p); p += align_up(cap * 8, 256);
     w->f = (int32_t*)(base + p); p += align_up(cap * 4, 256);
+    w->ef = (int32_t*)(base + p); p += align_up(cap * 4, 256);
+    w->eB = (uint32_t*)(base + p); p += align_up(cap * 4, 256);
+    w->ec = (uint32_t*)(base + p); p += align_up(cap * 4, 256);
+    w->handoff = (int*)(base + p); p += 256;
     w->flags = (AdmitFlags*)(base + p); p += 256;
     w->total = p;
 }
@@ -219,9 +328,16 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     rc = sort_u64(w.rsort, w.r0, w.r1, w.r0, n_run, 32, 64, st, &g_launches_admit);
     if (rc) return SVF_ECUDA;
     // a4 + a5
+    const bool slots = M < ((int64_t)1 << 30);        // 32-bit wrapping arithmetic of the slot passes is exact
     k_admit<<<1, ADMIT_THREADS, 0, st>>>(M, t, n_wait, w_s, w_o, n_run, r_kv, r_rem, w.wsort.plan, w.rsort.plan,
-                                         w.flags, w.f, w.A, n_admitted_out, admitted_idx_out, status_out);
+                                         w.flags, w.f, w.A, n_admitted_out, admitted_idx_out, status_out,
+                                         slots ? w.handoff : nullptr);
     ++g_launches_admit;
+    if (slots) {
+        k_admit_slots<256><<<1, 256, 0, st>>>(M, n_wait, w_s, w_o, n_run, r_kv, w.wsort.plan, w.rsort.plan, w.handoff,
+                                              w.f, w.A, w.ef, w.eB, w.ec, n_admitted_out, admitted_idx_out, status_out);
+        ++g_launches_admit;
+    }
     if (sorted_words_out) {
         rc = sort_result_to(w.wsort, sorted_words_out, n_wait, st, &g_launches_admit);
         if (rc) return SVF_ECUDA;

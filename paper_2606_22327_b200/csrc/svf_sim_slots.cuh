@@ -248,6 +248,34 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #define SVF_PUT8(ik, OP, k0)  if ((ik) & 4) { SVF_PUT4(ik, OP, k0 + 4) } else { SVF_PUT4(ik, OP, k0) }
 #define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
 
+// The per-slot operations of the passes.  They are macros over the LOCAL names of the calling
+// kernel (k_sim_slots here, k_admit_slots in svf_admit.cu): slots f[], B[], c[]; the head's t1 =
+// t + 1, oh = o_h, fh / fhu = f_h, Kc = s_h - t - M, add = s_h - t; accumulators acc, viol, dm
+// (evaluation) and wmax, minge (blocked head); cntE / cntU under COUNT.
+#define SVF_EVAL(k) {                                                                          \
+    const uint32_t x = (uint32_t)f[k] - t1;                            \
+    if (f[k] >= fh) acc += c[k] + fhu;                                 \
+    if (x < oh) {                                                      \
+        viol = __viaddmax_s32((int)B[k], (int)Kc, viol);               \
+        B[k] += add + (uint32_t)f[k];                                  \
+        if (COUNT) cntU += 1;                                          \
+    }                                                                  \
+    dm = __funnelshift_l(x, dm, 1);                                    \
+    if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
+}
+#define SVF_BLOCK(k) {                                                                         \
+        const uint32_t x = (uint32_t)f[k] - t1;                        \
+        if (x < oh) {                                                  \
+            B[k] -= add + (uint32_t)f[k];                              \
+            const int v = (int)(B[k] + Kc), d = (int)x + 1;            \
+            const int w = v < d ? v : d;                               \
+            wmax = w > wmax ? w : wmax;                                \
+            if (COUNT) cntU -= 1;                                      \
+        }                                                              \
+        if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
+    }
+#define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
+
 template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
 __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
 {
@@ -464,19 +492,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
                         const int g4 = (kmax + 3) >> 2;
                         const bool use_ext = hw > REGCAP;
-#define SVF_EVAL(k) {                                                                          \
-                            const uint32_t x = (uint32_t)f[k] - t1;                            \
-                            if (f[k] >= fh) acc += c[k] + fhu;                                 \
-                            if (x < oh) {                                                      \
-                                viol = __viaddmax_s32((int)B[k], (int)Kc, viol);               \
-                                B[k] += add + (uint32_t)f[k];                                  \
-                                if (COUNT) cntU += 1;                                          \
-                            }                                                                  \
-                            dm = __funnelshift_l(x, dm, 1);                                    \
-                            if (COUNT) cntE += (long long)((x >> 31) ^ 1u);                    \
-                        }
                         SVF_SLOT_GROUPS(g4, SVF_EVAL)
-#undef SVF_EVAL
                         // lowest free register slot of this thread as a one-hot bit (bit k of dm =
                         // slot k is dead); the group takes the lowest (slot, thread) pair
                         const uint32_t low = dm ? (dm & (0u - dm)) : (1u << (4 * g4));
@@ -503,19 +519,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             // ---- blocked (no bypass): take the update back and find how
                             // long the head stays blocked at least --------------------------------
                             int wmax = 0, minge = INT_MAX;
-#define SVF_BLOCK(k) {                                                                         \
-                                const uint32_t x = (uint32_t)f[k] - t1;                        \
-                                if (x < oh) {                                                  \
-                                    B[k] -= add + (uint32_t)f[k];                              \
-                                    const int v = (int)(B[k] + Kc), d = (int)x + 1;            \
-                                    const int w = v < d ? v : d;                               \
-                                    wmax = w > wmax ? w : wmax;                                \
-                                    if (COUNT) cntU -= 1;                                      \
-                                }                                                              \
-                                if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
-                            }
                             SVF_SLOT_GROUPS(g4, SVF_BLOCK)
-#undef SVF_BLOCK
                             if (use_ext) {
                                 for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                     const int e = q - REGCAP;
@@ -546,9 +550,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             const int ik = 31 - __clz(fkey >> TSHIFT);           // uniform
                             const bool mine = (fkey & (THREADS - 1)) == tid;
                             idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
-#define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
                             SVF_PUT16(ik, SVF_PUT)
-#undef SVF_PUT
                         } else {
                             // every register slot is live: the lowest dead ext slot, else a new one
                             if (use_ext) {

@@ -351,13 +351,21 @@ def _admit_both(B, oracle, policy, M, st, O0=179, O1=887):
 
 
 @pytest.mark.parametrize("n_wait,n_run", [(0, 0), (0, 50), (1, 0), (37, 0), (1024, 256), (5000, 1024),
-                                           (5001, 1024), (70_000, 4096), (1 << 18, 300)])
+                                           (5001, 1024), (70_000, 4096), (1 << 18, 300), (3000, 6000)])
 def test_admit_matches_oracle(B, oracle, n_wait, n_run):
-    M = 1_000_000
+    M = 1_000_000 if n_run <= 4096 else 6_000_000        # (3000, 6000): beyond the 4096 register slots
     st = _admit_state(n_wait + n_run, n_wait, n_run, M)
     ks = [_admit_both(B, oracle, policy, M, st) for policy in range(4)]
     if n_wait >= 1024 and n_run <= 1024:
         assert max(ks) > 0
+
+
+def test_admit_wide_budget_takes_the_sorted_array_kernel(B, oracle):
+    """M >= 2^30: the 32-bit slot passes are not exact any more; the 64-bit sorted-array path runs."""
+    st = _admit_state(77, 4000, 500, 1_000_000)
+    for M in ((1 << 30) - 1, 1 << 30, 5 << 30):
+        k = _admit_both(B, oracle, 0, M, st)
+        assert k == 4000                                  # everything fits
 
 
 def test_admit_everything_fits_and_nothing_fits(B, oracle):
