@@ -1,4 +1,4 @@
-// The register-resident simulator kernel (a4-a7), included by svf_simulate.cu only.
+// The register-resident simulator kernel (a4-a7), included by svf_simulate.cu; svf_admit.cu reuses its slot passes.
 //
 // RUNNING SET as unordered SLOTS.  Slot j of an instance holds, for one request in flight,
 //     f_j   absolute finish step (int32); the slot is DEAD (free) once f_j <= t (0 = never used)

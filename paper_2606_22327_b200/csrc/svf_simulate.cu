@@ -1,21 +1,22 @@
 // a1-a7: the batched discrete-time simulator of the paper's KV-cache model under the
 // SVF / 1-bit SVF / SJF / FCFS admission rule (Alg. 1 Process 2).
 //
-// Phase A (device-wide, HBM-bound):  k_sim_pack  keys (Eq. 1 / Eq. 2) packed as
-//     [ instance | key (32) | local id (sb) ]  ->  onesweep radix sort on [sb, sb+32+ib)
-//     (stable, input is in (instance, arrival, id) order, so the result is the
-//     (instance, key, arrival, id) order)  ->  k_sim_rank  order[] / rank[] per instance.
-// Phase B (persistent, on-chip):  k_sim  one thread group (warp or CTA) per instance, work
-//     handed out by an atomic counter; running set and waiting bitmap in shared memory (in an
-//     L2-resident workspace slot when an instance is too large), see svf_state.cuh.
-// Phase C:  p99 by one more onesweep sort of (instance, latency) words + k_sim_p99.
+// Phase A (presort, HBM-bound): the priority order of every instance under every policy of the
+//     call.  Instances of at most 4096 requests: k_seg_sort, one CTA per instance, keys (Eq. 1 /
+//     Eq. 2) + stable radix passes + rank entirely in shared memory (svf_sort.cu).  Larger ones:
+//     k_sim_pack  keys packed as [ instance | key (32) | local id (sb) ]  ->  device-wide onesweep
+//     on [sb, sb+32+ib) (stable; input in (instance, arrival, id) order, so the result is the
+//     (instance, key, arrival, id) order)  ->  k_sim_rank  order[] / rank[] / records.
+// Phase B (persistent, on-chip):  k_sim_slots (svf_sim_slots.cuh)  one thread group (warp or CTA)
+//     per (policy, instance) work item, handed out by an atomic counter; running set in registers,
+//     waiting bitmap and records in registers / shared memory; validates the data, simulates,
+//     selects p99.  For M >= 2^30 (32-bit slot arithmetic not exact): k_sim below, sorted (f, A)
+//     arrays in shared memory in 64 bit, one policy per launch, p99 by one more onesweep sort
+//     (phase C).
 //
 // Time advance is event driven but exact (R1, R16): steps on which nothing can happen are
-// jumped over -- an empty queue jumps to the next arrival/completion; a blocked head jumps to
-// the next arrival/completion or to the first step at which condition (2) of the check can
-// hold (it relaxes by exactly one token per step while the running set is unchanged) -- and
-// the skipped steps are still counted into rounds/decisions exactly as the step-by-step
-// definition counts them.
+// jumped over and still counted into rounds/decisions exactly as the step-by-step definition
+// counts them (closed forms in the header of svf_sim_slots.cuh).
 #include <limits.h>
 
 #include "svf_internal.cuh"

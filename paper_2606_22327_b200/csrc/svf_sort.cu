@@ -545,12 +545,8 @@ int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const 
     // items per thread sized to the largest instance (registers: occupancy of small segments)
 #define SVF_SEG_LAUNCH(IPT)                                                                             \
     do {                                                                                                \
-        static bool attr_set = false;                                                                   \
-        if (!attr_set) {                                                                                \
-            cudaFuncSetAttribute(k_seg_sort<IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
-                                 2 * SEG_SORT_MAX * (int)sizeof(uint64_t));                             \
-            attr_set = true;                                                                            \
-        }                                                                                               \
+        cudaFuncSetAttribute(k_seg_sort<IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                             2 * SEG_SORT_MAX * (int)sizeof(uint64_t));   /* per device: set every time */ \
         int per_sm = 0;                                                                                 \
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort<IPT>, SORT_THREADS, smem) \
                 != cudaSuccess || per_sm < 1)                                                           \
