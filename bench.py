@@ -62,6 +62,7 @@ def parse_args():
     ap.add_argument("--instances", type=int, default=4096)
     ap.add_argument("--requests", type=int, default=1000)
     ap.add_argument("--lam", type=float, default=4.0)
+    ap.add_argument("--e2e-chunks", type=int, default=4, help="instance chunks (streams) of the end-to-end leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel and per-config extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -278,20 +279,34 @@ def run_ours(args):
              "phase_c_p99": float(phase[:, 2].sum() / phase[:, 3].sum())}
 
     # ---- end to end through the C ABI with host buffers: H2D of the trace from pinned memory,
-    # the four policy runs, D2H of every output --------------------------------------------------
-    pinned = {k: torch.from_numpy(getattr(batch, k)).pin_memory() for k in ("offsets", "arrival", "prompt", "output", "bit")}
-    host_out = [{k: torch.empty_like(getattr(o, k), device="cpu").pin_memory() for k in B.RESULT_FIELDS} for o in outs]
-    h2d = sum(int(v.numel() * v.element_size()) for v in pinned.values())
-    d2h = sum(int(v.numel() * v.element_size()) for ho in host_out for v in ho.values())
+    # the four policy runs, D2H of every output.  The batch goes through in `--e2e-chunks` chunks of
+    # instances, each on its own stream (copies of one chunk overlap the simulation of the other);
+    # per chunk it is the same public call as above --------------------------------------------
+    n_chunks = max(1, min(args.e2e_chunks, batch.n_instances))
+    bounds = [S.strong_shard(batch.n_instances, c, n_chunks) for c in range(n_chunks)]
+    subs = [batch.subset(range(lo, hi)) for lo, hi in bounds]
+    streams = [torch.cuda.Stream(device=dev) for _ in range(n_chunks)]
+    pinned, c_outs, c_ws, host_out = [], [], [], []
+    for sub in subs:
+        pinned.append({k: torch.from_numpy(getattr(sub, k)).pin_memory() for k in ("offsets", "arrival", "prompt", "output", "bit")})
+        dsub = B.DeviceTrace.from_host(sub, device=dev)
+        c_outs.append([B.SimOut.alloc(dsub) for _ in POLICIES])
+        c_ws.append(torch.empty(B.svf_simulate_policies_workspace_bytes(dsub, len(POLICIES)), dtype=torch.uint8, device=dev))
+        host_out.append([{k: torch.empty_like(getattr(o, k), device="cpu").pin_memory() for k in B.RESULT_FIELDS}
+                         for o in c_outs[-1]])
+    h2d = sum(int(v.numel() * v.element_size()) for pc in pinned for v in pc.values())
+    d2h = sum(int(v.numel() * v.element_size()) for hc in host_out for ho in hc for v in ho.values())
 
     def e2e_step():
-        d = B.DeviceTrace.from_host(batch, device=dev, pinned=pinned, non_blocking=True)
-        B.svf_simulate_policies(d, POLICIES, outs=outs, ws=ws)
-        for i in range(len(POLICIES)):
-            for k in B.RESULT_FIELDS:
-                host_out[i][k].copy_(getattr(outs[i], k), non_blocking=True)
+        for c in range(n_chunks):
+            with torch.cuda.stream(streams[c]):
+                d = B.DeviceTrace.from_host(subs[c], device=dev, pinned=pinned[c], non_blocking=True)
+                B.svf_simulate_policies(d, POLICIES, outs=c_outs[c], ws=c_ws[c])
+                for i in range(len(POLICIES)):
+                    for k in B.RESULT_FIELDS:
+                        host_out[c][i][k].copy_(getattr(c_outs[c][i], k), non_blocking=True)
         torch.cuda.synchronize()
-        return int(host_out[0]["total_latency"][0])
+        return int(host_out[0][0]["total_latency"][0])
 
     e2e_step()
     barrier()
@@ -335,7 +350,7 @@ def run_ours(args):
         "step_ms": step_ms,
         "clocks": clocks,
         "e2e": {"value": rs_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": 1e3 * e2e_s},
+                "ms_per_step": 1e3 * e2e_s, "chunks": n_chunks},
         "gpu_launches": launches_all,
         "roofline": {"kernel": "k_sim_slots (persistent simulator, phase B)", "bound": "alu",
                      "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "Tlane-op/s",
