@@ -330,7 +330,7 @@ def run_ours(args):
     # ---- algorithmic work of the dominant kernel, counted by its counting variant (untimed) ----
     B.set_profiling(2)
     B.svf_simulate_policies(dt_dev, POLICIES, outs=outs, ws=ws)
-    E, U = B.simulate_work_counts()
+    E, U, n_eval, n_blocked = B.simulate_work_counts()
     B.set_profiling(False)
     ops_per_launch = OPS_PER_EXAMINED * E + OPS_PER_UPDATED * U
 
@@ -359,6 +359,7 @@ def run_ours(args):
                      "algorithmic_ops_per_launch": ops_per_launch,
                      "entries_examined_per_launch": E,
                      "entries_updated_per_launch": U,
+                     "evaluations_per_launch": n_eval, "blocked_evaluations_per_launch": n_blocked,
                      "kernel_ms": sim_ms, "share_of_step": share,
                      "hbm": {"algorithmic_bytes_per_launch": sim_bytes,
                              "achieved_gbs": sim_bytes / (sim_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,

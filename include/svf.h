@@ -176,10 +176,10 @@ int64_t svf_last_launch_count(int which);
  * kernel), [3] the whole call.  Returns SVF_EINVAL if profiling was off.
  * svf_set_profiling(2): as 1, and the simulator kernel also counts its algorithmic work (a
  * slower variant of the same kernel, same results; M < 2^30 only): svf_simulate_work_counts
- * synchronises and writes counts_out ([host] uint64[2]): [0] E = running entries examined,
+ * synchronises and writes counts_out ([host] uint64[4]): [0] E = running entries examined,
  * summed over every head evaluation (a4), [1] U = running entries updated, summed over every
- * admission (a5).  The counts live in the workspace of that call, which must still be
- * allocated.  svf_set_profiling(0) switches both off. */
+ * admission (a5), [2] head evaluations performed, [3] of them blocked.  The counts live in the
+ * workspace of that call, which must still be allocated.  svf_set_profiling(0) switches both off. */
 void svf_set_profiling(int mode);
 int svf_simulate_phase_ms(float* ms_out);
 int svf_simulate_work_counts(uint64_t* counts_out);

@@ -117,11 +117,12 @@ def set_profiling(mode) -> None:
 
 
 def simulate_work_counts():
-    """(E, U) of the last svf_simulate call made under set_profiling(2): running entries examined
-    over all head evaluations, running entries updated over all admissions."""
-    buf = (C.c_uint64 * 2)()
+    """(E, U, evaluations, blocked) of the last svf_simulate call made under set_profiling(2): running
+    entries examined over all head evaluations, running entries updated over all admissions, head
+    evaluations performed, and how many of them found the head blocked."""
+    buf = (C.c_uint64 * 4)()
     _check(lib().svf_simulate_work_counts(buf), "svf_simulate_work_counts")
-    return int(buf[0]), int(buf[1])
+    return tuple(int(x) for x in buf)
 
 
 def simulate_phase_ms():

@@ -142,7 +142,7 @@ struct SlotArgs {
     int n_policies;
     PolicyIO io[MAX_POLICIES];
     unsigned long long* work_ctr;
-    unsigned long long* work_counts; // [2] E, U (only written by the COUNT variant)
+    unsigned long long* work_counts; // [4] E, U, evaluations, blocked evaluations (COUNT variant only)
     char* gstate; size_t slot_bytes; // per-CTA state when it does not fit in shared memory
     int ecap;                        // ext slots per instance
     int qcap;                        // bitmap capacity (ranks)
@@ -357,6 +357,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
         int mk = 0, peak = 0;
         uint32_t rounds = 0, decisions = 0;
         long long cntE = 0, cntU = 0;
+        unsigned long long cntV = 0, cntBk = 0;   // uniform: evaluations, blocked evaluations
         int64_t p99v = 0;
 
         if (status != SVF_OK || n == 0) {
@@ -514,11 +515,13 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
                             }
                         }
                         reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
+                        if (COUNT) ++cntV;
                         const int Ah = head.s + head.o + (int)acc;        // exact: 0 <= A_h <= 2M < 2^31
                         if (viol > 0 || Ah > Mi) {
                             // ---- blocked (no bypass): take the update back and find how
                             // long the head stays blocked at least --------------------------------
                             int wmax = 0, minge = INT_MAX;
+                            if (COUNT) ++cntBk;
                             SVF_SLOT_GROUPS(g4, SVF_BLOCK)
                             if (use_ext) {
                                 for (int q = REGCAP + tid; q < hw; q += THREADS) {
@@ -626,6 +629,7 @@ __global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
             if (lane == 0 && g.work_counts) {
                 atomicAdd(&g.work_counts[0], (unsigned long long)cntE);
                 atomicAdd(&g.work_counts[1], (unsigned long long)cntU);
+                if (wrp == 0) { atomicAdd(&g.work_counts[2], cntV); atomicAdd(&g.work_counts[3], cntBk); }
             }
         }
         if (wrp == 0) {

@@ -685,7 +685,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
     const bool count = g_profiling == 2;
     if (count) {
-        if (cudaMemsetAsync(w.counts, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
+        if (cudaMemsetAsync(w.counts, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
         g_counts_dev = w.counts;
     }
 #define SVF_SLOTS_LAUNCH(T, S, Q)                                                         \
@@ -796,9 +796,9 @@ extern "C" void svf_set_profiling(int mode) { g_profiling = mode == 2 ? 2 : (mod
 extern "C" int svf_simulate_work_counts(uint64_t* counts_out)
 {
     if (!counts_out || !g_counts_dev) return SVF_EINVAL;
-    unsigned long long h[2] = {0, 0};
+    unsigned long long h[4] = {0, 0, 0, 0};
     if (cudaMemcpy(h, g_counts_dev, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return SVF_ECUDA;
-    counts_out[0] = h[0]; counts_out[1] = h[1];
+    for (int k = 0; k < 4; ++k) counts_out[k] = h[k];
     return SVF_OK;
 }
 
