@@ -484,3 +484,33 @@ def test_more_running_requests_than_register_slots(B, oracle):
         # the point of the case: most of an instance runs at once
         started_early = (ref.start[: tr.offsets[1]] < 150).sum()
         assert started_early > 0.6 * n
+
+
+@pytest.mark.parametrize("rnd", range(8))
+def test_fuzz_random_batches(B, oracle, rnd):
+    """Seeded random batches over the whole parameter space of the kernels: instance sizes 0..2500
+    (warp kernel, CTA kernels), arrival spreads 0..300, budgets from barely one request to hundreds
+    of requests (blocked heads, ext slots), predicted keys on odd rounds, 1..4 policies per call."""
+    sd = T.instance_seed(55, rnd)
+    u = lambda stream, lo, hi: int(T.uniform_int(sd, stream, 1, lo, hi)[0])
+    sc = (1, 10, 3)[rnd % 3]
+    s_hi, o_hi = u(1, 1, 40 * sc), u(2, 1, 60 * sc)
+    M = u(3, s_hi + o_hi, (6 if sc == 1 else 400) * (s_hi + o_hi) + 5)
+    nmax = (12, 60, 300, 1100, 2500)[u(4, 0, 4)]
+    I = 40 if nmax > 300 else u(5, 200, 1500)
+    parts = []
+    for i in range(I):
+        si = T.instance_seed(56, rnd * 100_000 + i)
+        n = int(T.uniform_int(si, 1, 1, 0, nmax)[0])
+        a_hi = (0, 3, 30, 300)[int(T.uniform_int(si, 2, 1, 0, 3)[0])]
+        parts.append(T.random_small(rnd * 100_000 + i, n, s_hi, o_hi, M, a_hi=a_hi, O0=1 + rnd, O1=7 + 5 * rnd))
+    tr = T.concat(parts, f"fuzz{rnd}", M, 1 + rnd, 7 + 5 * rnd)
+    if rnd % 2:
+        tr = T.with_predicted_lengths(tr, sigma=0.7, seed=rnd, hi=max(2, 3 * o_hi))
+    pols = [(rnd + k) % 4 for k in range(1 + rnd % 4)]
+    import torch
+    outs = B.svf_simulate_policies(B.DeviceTrace.from_host(tr), pols)
+    torch.cuda.synchronize()
+    for pol, out in zip(pols, outs):
+        ref = oracle.simulate(tr, pol, n_threads=8)
+        assert_same({k: getattr(out, k).cpu().numpy() for k in FIELDS}, ref, tr, f"fuzz {rnd} policy {pol}")
