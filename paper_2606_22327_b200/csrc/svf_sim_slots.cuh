@@ -276,8 +276,12 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     }
 #define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
 
+// Register budget of the warp kernel: without a bound ptxas takes 127 registers (16 warps per SM);
+// asked for 19 CTAs per SM it fits the kernel into 96 registers WITHOUT spills (21 warps per SM
+// resident) and the launch is 5 % faster; 20 also gives 96 registers but a slower schedule, 17-18
+// and 21 spill (all measured on configs[2], profiles/r01_kslots_full.md).
 template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
-__global__ void __launch_bounds__(THREADS) k_sim_slots(SlotArgs g)
+__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_sim_slots(SlotArgs g)
 {
     static_assert(K == 16, "SVF_SLOT_GROUPS / SVF_PUT16 are written out for 16 register slots per thread");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
