@@ -50,7 +50,7 @@ OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
 SIM_BYTES_PER_REQUEST = 36
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/r01_kslots_full.md (one launch = four policies)
-SIM_DRAM_TRAFFIC_BYTES = 492.0e6
+SIM_DRAM_TRAFFIC_BYTES = 515.1e6
 
 
 def parse_args():
