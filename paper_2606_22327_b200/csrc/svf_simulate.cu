@@ -380,7 +380,13 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     int64_t w = I > 0 ? target_warps / (I * (P > 0 ? P : 1)) : 1;   // P policies share one launch
     int threads = 32;
     const int tmax = c.slots ? 256 : 1024;
-    while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
+    // a group wider than 128 threads only pays when the running set can outgrow 128 x 16 register
+    // slots; it is at most mx and, at a few hundred tokens per running request, about M / 512
+    // (measured: configs[3] 190 vs 201 ms, configs[4] 5.6 vs 10.9 ms with 128 instead of 256 threads)
+    const int64_t r_est = c.slots ? (mx < M / 512 ? mx : M / 512) : mx;
+    while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx &&
+           (threads < 128 || r_est > (int64_t)threads * SLOT_K))
+        threads *= 2;
     if (threads == 64) threads = 128;
     if (threads == 512) threads = 1024;
     c.gslot_bytes = 0; c.max_cta_per_sm = 2;

@@ -221,7 +221,7 @@ def test_random_small_instances_all_policies(B, oracle):
 
 
 def test_group_widths_and_state_placement(B, oracle):
-    """Shapes that select each kernel variant: 32/128/256/1024 threads, shared/global state."""
+    """Shapes that select the warp kernel and the CTA kernels (the 256-thread one: see the crowd test)."""
     shapes = [(4096 // 8, 40, 2.0),     # many small instances -> one warp each
               (100, 600, 4.0),         # 128 threads
               (1, 2000, 4.0),          # 256 threads
