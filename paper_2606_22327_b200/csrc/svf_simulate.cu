@@ -374,21 +374,24 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.cap = (int)((mx + 31) / 32 * 32);
     c.slots = M < ((int64_t)1 << 30);
     c.ecap = 0; c.qcap = c.cap; c.qreg = false;
-    // group width: enough warps in flight to cover the GPU (about 16 per SM), no wider than the
-    // running set can use
+    // group width.  Register-slot kernels: one WARP per item (512 register slots) unless the running
+    // set can outgrow them and there are warps to spare: R is at most mx and, at a few hundred
+    // tokens per running request, about M / 512.  Measured: a CTA-wide group is slower than a warp
+    // whenever the set fits the warp's registers (one more barrier and a replicated scalar part per
+    // evaluation); 128 threads beat 256 until R passes 2048 (configs[3] 190 vs 201 ms, configs[4]
+    // 5.6 vs 10.9 ms).  The wide 64-bit kernel keeps the occupancy rule (about 16 warps per SM).
     const int64_t target_warps = (int64_t)sm_count() * 16;
     int64_t w = I > 0 ? target_warps / (I * (P > 0 ? P : 1)) : 1;   // P policies share one launch
     int threads = 32;
-    const int tmax = c.slots ? 256 : 1024;
-    // a group wider than 128 threads only pays when the running set can outgrow 128 x 16 register
-    // slots; it is at most mx and, at a few hundred tokens per running request, about M / 512
-    // (measured: configs[3] 190 vs 201 ms, configs[4] 5.6 vs 10.9 ms with 128 instead of 256 threads)
-    const int64_t r_est = c.slots ? (mx < M / 512 ? mx : M / 512) : mx;
-    while (threads < tmax && (threads * 2) / 32 <= w && threads * 4 <= mx &&
-           (threads < 128 || r_est > (int64_t)threads * SLOT_K))
-        threads *= 2;
-    if (threads == 64) threads = 128;
-    if (threads == 512) threads = 1024;
+    if (c.slots) {
+        const int64_t r_est = mx < M / 512 ? mx : M / 512;
+        if (r_est > 32 * SLOT_K && w >= 4) threads = 128;
+        if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
+    } else {
+        while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
+        if (threads == 64) threads = 128;
+        if (threads == 512) threads = 1024;
+    }
     c.gslot_bytes = 0; c.max_cta_per_sm = 2;
     if (c.slots) {
         auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };

@@ -222,7 +222,8 @@ def test_random_small_instances_all_policies(B, oracle):
 
 def test_group_widths_and_state_placement(B, oracle):
     """Shapes that select the warp kernel and the CTA kernels (the 256-thread one: see the crowd test)."""
-    shapes = [(4096 // 8, 40, 2.0),     # many small instances -> one warp each
+    shapes = [(200, 1300, 4.0),        # one warp each, shared-memory bitmap (more than 1024 requests)
+              (4096 // 8, 40, 2.0),     # many small instances -> one warp each
               (100, 600, 4.0),         # 128 threads
               (1, 2000, 4.0),          # 256 threads
               (2, 9000, 8.0)]          # 1024 threads, shared state
