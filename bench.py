@@ -62,7 +62,7 @@ def parse_args():
     ap.add_argument("--instances", type=int, default=4096)
     ap.add_argument("--requests", type=int, default=1000)
     ap.add_argument("--lam", type=float, default=4.0)
-    ap.add_argument("--e2e-chunks", type=int, default=4, help="instance chunks (streams) of the end-to-end leg")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="instance chunks (streams) of the end-to-end leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel and per-config extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
