@@ -45,7 +45,7 @@ typedef enum {
     SVF_EINVAL = 1,       /* host: null pointer, negative size, unknown policy, O0/O1 < 1, missing bit */
     SVF_EWORKSPACE = 2,   /* host: ws is NULL or ws_bytes too small                                   */
     SVF_ECUDA = 3,        /* host: no device / launch failed (cudaGetLastError != success)           */
-    SVF_ERANGE = 16,      /* data: o_i < 1, s_i < 0 or a_i < 0 (running set: rem < 1 or kv < 0)        */
+    SVF_ERANGE = 16,      /* data: o_i < 1, s_i < 0, a_i < 0 or output_key_i < 1 (running set: rem < 1 or kv < 0) */
     SVF_EUNSORTED = 17,   /* data: arrivals decrease inside an instance                              */
     SVF_EINFEASIBLE = 18, /* data: s_i + o_i > M, could never be admitted (paper assumes <= aM) */
     SVF_EOVERFLOW = 19    /* data: key >= 2^32, or max a + sum o >= 2^31 (horizon bound)       */
