@@ -240,7 +240,8 @@ def test_policies_in_one_call(B, oracle):
     cases = [(T.config3(n_instances=300, n=200, lam=4.0, M=60_000), None, [0, 1, 2, 3]),
              (T.config3(n_instances=6, n=1500, lam=8.0, M=60_000), None, [3, 0, 2]),
              (T.config5(n_instances=3, n=5000, M=200_000, p_flip=0.2), None, [1, 0]),
-             (T.config3(n_instances=20, n=100, lam=4.0), 1 << 30, [0, 3])]
+             (T.config3(n_instances=20, n=100, lam=4.0), 1 << 30, [0, 3]),
+             (T.config3(n_instances=70, n=150, lam=8.0, M=40_000), None, [0, 1, 2, 3, 3, 2, 1, 0])]   # the maximum of 8
     for tr, M, pols in cases:
         dt = B.DeviceTrace.from_host(tr)
         outs = B.svf_simulate_policies(dt, pols, M)
