@@ -79,7 +79,8 @@ int svf_ref_keys(int policy, int64_t n, const int32_t *s, const int32_t *o, cons
                  const uint8_t *bit, int32_t O0, int32_t O1, uint64_t *words_out)
 {
     if (policy < 0 || policy > 3 || n < 0) return ST_EINVAL;
-    if (policy == POL_SVF_1BIT && (!bit || O0 < 1 || O1 < 1)) return ST_EINVAL;
+    /* boundary rule (include/svf.h, "bit"): the bit array is required only when there is a request to read it for */
+    if (policy == POL_SVF_1BIT && ((n > 0 && !bit) || O0 < 1 || O1 < 1)) return ST_EINVAL;
     int rc = ST_OK;
     for (int64_t i = 0; i < n; ++i) {
         int64_t k = ref_key(policy, s[i], o[i], a ? a[i] : 0, bit ? bit[i] : 0, O0, O1);
@@ -184,7 +185,7 @@ int svf_ref_admit(int policy, int64_t M, int32_t t, int feas_mode,
 {
     (void)t; /* the check is relative to "now"; t only dates the decision */
     if (policy < 0 || policy > 3 || n_wait < 0 || n_run < 0 || M < 0) return ST_EINVAL;
-    if (policy == POL_SVF_1BIT && (!w_bit || O0 < 1 || O1 < 1)) return ST_EINVAL;
+    if (policy == POL_SVF_1BIT && ((n_wait > 0 && !w_bit) || O0 < 1 || O1 < 1)) return ST_EINVAL;
     for (int64_t i = 0; i < n_wait; ++i) {
         if (w_o[i] < 1 || w_s[i] < 0 || w_a[i] < 0) return ST_ERANGE;
         if (i > 0 && w_a[i] < w_a[i - 1]) return ST_EUNSORTED;
@@ -371,7 +372,7 @@ int svf_ref_simulate_pred(int64_t n_instances, const int64_t *offsets, const int
                           int64_t *decisions, int32_t *status)
 {
     if (n_instances < 0 || policy < 0 || policy > 3 || M < 0) return ST_EINVAL;
-    if (policy == POL_SVF_1BIT && (!bit || O0 < 1 || O1 < 1)) return ST_EINVAL;
+    if (policy == POL_SVF_1BIT && ((n_instances > 0 && offsets[n_instances] > 0 && !bit) || O0 < 1 || O1 < 1)) return ST_EINVAL;
     if (n_threads < 1) n_threads = 1;
 #ifdef _OPENMP
 #pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads)
@@ -410,8 +411,8 @@ int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t 
  * NEXT-2: the volume lower bound of Proposition 3.1 (Eq. 5) for burst input,
  *     M * TEL(OPT) >= LB = sum_{j=1..N} sum_{i=1..j} vol_(i),   vol_(1) <= ... <= vol_(N),
  * written as printed: sort the volumes (Eq. 1), then for every j add the sum of the first j.
- * lb_out[j] = LB of instance j (int64); status_out[j] = ST_EOVERFLOW if LB >= 2^63 (lb 0),
- * ST_ERANGE if some o < 1 or s < 0.  Arrivals are not looked at: the bound is about the burst
+ * lb_out[j] = LB of instance j (int64); status_out[j] = ST_EOVERFLOW if LB >= 2^63 or some volume
+ * >= 2^32 (lb 0; R11: the width rule of every key), ST_ERANGE if some o < 1 or s < 0 (wins).  Arrivals are not looked at: the bound is about the burst
  * version of the instance.
  * ---------------------------------------------------------------------------------------- */
 int svf_ref_volume_lower_bound(int64_t n_instances, const int64_t *offsets, const int32_t *prompt,
@@ -425,6 +426,8 @@ int svf_ref_volume_lower_bound(int64_t n_instances, const int64_t *offsets, cons
         for (int64_t i = 0; i < n; ++i) {
             if (output[lo + i] < 1 || prompt[lo + i] < 0) st = ST_ERANGE;
             vol[i] = ref_key(POL_SVF, prompt[lo + i], output[lo + i], 0, 0, 0, 0);
+            /* a volume is an SVF key: keys >= 2^32 are ST_EOVERFLOW at every entry point (reading R11) */
+            if (st == ST_OK && vol[i] >= ((int64_t)1 << 32)) st = ST_EOVERFLOW;
         }
         unsigned __int128 lb = 0, prefix = 0;
         if (st == ST_OK) {

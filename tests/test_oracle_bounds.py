@@ -159,6 +159,16 @@ def test_volume_lower_bound_closed_forms(oracle):
     bad = T.random_small(3, 5, 9, 9, 50)
     bad.output[2] = 0
     assert int(oracle.volume_lower_bound(bad)[1][0]) == oracle.ERANGE
+    # a volume is an SVF key: >= 2^32 is EOVERFLOW at every entry point (reading R11), the same rule as
+    # in keys / simulate.  s = o = 60,000: 60000^2 + 60000*60001/2 = 5,400,030,000 >= 2^32 = 4,294,967,296;
+    # s = 30,000, o = 60,000: 3,600,030,000 < 2^32
+    below = T._one("below", np.zeros(2, np.int32), np.array([30_000, 30_000]), np.array([60_000, 60_000]), np.zeros(2, np.uint8), 10 ** 9, 1, 1)
+    lb, st = oracle.volume_lower_bound(below)
+    assert int(st[0]) == 0 and int(lb[0]) == 3 * 3_600_030_000
+    mixed = T._one("mixed", np.zeros(2, np.int32), np.array([60_000, 30_000]), np.array([60_000, 60_000]), np.zeros(2, np.uint8), 10 ** 9, 1, 1)
+    lb, st = oracle.volume_lower_bound(mixed)
+    assert int(st[0]) == oracle.EOVERFLOW and int(lb[0]) == 0
+    assert oracle.keys(oracle.SVF, mixed.prompt, mixed.output)[0] == oracle.EOVERFLOW       # the same rule
 
 
 def test_volume_lower_bound_bounds_every_schedule_and_the_optimum(oracle):

@@ -45,6 +45,15 @@ def test_proxy_volume_and_comparator_keys(oracle):
     # 1-bit needs the bit array and proxies >= 1
     assert oracle.keys(oracle.SVF_1BIT, s, o, a, None, 2, 8)[0] == oracle.EINVAL
     assert oracle.keys(oracle.SVF_1BIT, s, o, a, bit, 0, 8)[0] == oracle.EINVAL
+    # ... but an array nobody would read may be missing: n = 0 (include/svf.h conventions)
+    e = np.zeros(0, np.int32)
+    assert oracle.keys(oracle.SVF_1BIT, e, e, e, None, 2, 8)[0] == oracle.OK
+    assert oracle.keys(oracle.SVF_1BIT, e, e, e, None, 0, 8)[0] == oracle.EINVAL
+    rc, idx, _ = oracle.admit(oracle.SVF_1BIT, 100, 0, e, e, e, None, 2, 8, [5], [3])
+    assert rc == oracle.OK and len(idx) == 0
+    empty = T._one("empty", e, e, e, np.zeros(0, np.uint8), 100, 2, 8)
+    empty.bit = None
+    assert int(oracle.simulate(empty, oracle.SVF_1BIT).status[0]) == oracle.OK
 
 
 @pytest.mark.parametrize("T_, b", [(16, 2), (81, 3), (256, 4)])
@@ -262,6 +271,75 @@ def test_admit_matches_simulator_first_step(oracle):
             rc2, idx2, _ = oracle.admit(policy, tr.M, 0, tr.prompt, tr.output, tr.arrival,
                                         tr.bit, tr.O0, tr.O1, [], [], mode=0)
             assert np.array_equal(idx, idx2)
+
+
+def test_admit_with_a_running_set_hand_states(oracle):
+    """svf_ref_admit with a NON-EMPTY running set, values derived by hand from Eq. 3c:
+    a running member (kv, rem) holds kv + d tokens d steps from now, d = 1..rem; a request
+    admitted now holds s + d for d = 1..o.
+    State 1: running (kv 6, rem 1), head (s 2, o 3), M = 9: d=1 holds 7 + 3 = 10 > 9 -> blocked.
+    State 2: running (kv 1, rem 6), same head: d=1..6 hold 2+3, 3+4, 4+5, 5, 6, 7 -> max 9 <= 9 ->
+    admitted.  The two states are each other with kv and rem swapped, so a swap anywhere in the
+    oracle's loading of the running set fails one of them.
+    State 3: running A (3, 2), B (1, 4); waiting x (s 2, o 1; vol 3), y (s 1, o 3; vol 9), SVF order
+    x, y.  With x: d=1 holds 4 + 2 + 3 = 9, d=2 holds 5 + 3 = 8.  With x and y: d=1 holds
+    4 + 2 + 3 + 2 = 11, d=2 holds 5 + 3 + 3 = 11, d=3 holds 4 + 4 = 8, d=4 holds 5.  So M = 8 admits
+    nobody, M = 9 and 10 admit x only, M = 11 admits both."""
+    z = np.zeros(1, np.int32)
+    for mode in (oracle.FEAS_LITERAL, oracle.FEAS_COMPLETION):
+        rc, idx, _ = oracle.admit(oracle.SVF, 9, 0, [2], [3], z, None, 1, 1, [6], [1], mode=mode)
+        assert rc == 0 and idx.tolist() == []
+        rc, idx, _ = oracle.admit(oracle.SVF, 9, 0, [2], [3], z, None, 1, 1, [1], [6], mode=mode)
+        assert rc == 0 and idx.tolist() == [0]
+        rc, idx, _ = oracle.admit(oracle.SVF, 8, 0, [2], [3], z, None, 1, 1, [1], [6], mode=mode)
+        assert rc == 0 and idx.tolist() == []                       # the boundary is inclusive: 9 > 8
+        for M, want in ((8, []), (9, [1]), (10, [1]), (11, [1, 0]), (50, [1, 0])):
+            # input order y, x (ids 0, 1): the priority order x, y is ids 1, 0
+            rc, idx, _ = oracle.admit(oracle.SVF, M, 7, [1, 2], [3, 1], [0, 0], None, 1, 1, [3, 1], [2, 4], mode=mode)
+            assert rc == 0 and idx.tolist() == want, (M, mode)
+
+
+@pytest.mark.parametrize("policy", [0, 2, 3])
+def test_admit_replays_simulator_states_with_running_sets(oracle, policy):
+    """The stateless call on states taken from a simulation of configs[1] (n = 2000): at step t
+    the running set is {i : k_i < t < k_i + o_i} with kv_i = s_i + t - k_i and rem_i = k_i + o_i - t
+    computed HERE from the definition (Eq. 3c), the waiting queue is {i : a_i <= t <=
+    k_i} in arrival order; the call must admit exactly the requests the simulator started at t, in
+    priority order, under both statements of FEASIBLE."""
+    tr = T.config2(1)
+    ref = oracle.simulate(tr, policy)
+    a, s, o = tr.arrival.astype(np.int64), tr.prompt.astype(np.int64), tr.output.astype(np.int64)
+    k = ref.start.astype(np.int64)
+    busy = np.unique(k[k > a])                         # steps that start somebody who had to wait
+    times = [int(busy[i]) for i in np.linspace(0, len(busy) - 1, 7).astype(int)] + [int(a[50]), 100, 450]
+    nonempty = 0
+    for t in times:
+        run = np.nonzero((k < t) & (k + o > t))[0]
+        wait = np.nonzero((a <= t) & (k >= t))[0]
+        kv, rem = s[run] + (t - k[run]), k[run] + o[run] - t
+        started = wait[k[wait] == t]
+        for mode in (oracle.FEAS_LITERAL, oracle.FEAS_COMPLETION):
+            rc, idx, words = oracle.admit(policy, tr.M, t, s[wait], o[wait], a[wait], tr.bit[wait], tr.O0, tr.O1,
+                                          kv, rem, mode=mode)
+            assert rc == 0
+            assert sorted(wait[idx].tolist()) == started.tolist(), (t, mode)
+            # admitted = a PREFIX of the priority order (no bypass, PAPER.md:507)
+            assert np.array_equal(words[: len(idx)] & np.uint64(0xFFFFFFFF), idx.astype(np.uint64))
+        nonempty += len(run) > 0 and len(started) > 0
+    assert nonempty >= 5
+
+
+def test_p99_is_the_nearest_rank_hand_values(oracle):
+    """Reading R13: p99 = the ceil(0.99 n)-th smallest latency.  With a budget that admits everybody
+    on arrival a request's latency is its o (Lemma G.1's equality case), so outputs 1..n in any order
+    give latencies 1..n and p99 = ceil(0.99 n): 1, 8, 99, 100 and 1980 for n = 2000."""
+    for n, want in ((1, 1), (8, 8), (100, 99), (101, 100), (199, 198), (200, 198), (2000, 1980)):
+        o = np.arange(1, n + 1, dtype=np.int32)
+        o = o[np.argsort(T.uniform(11, 3, n), kind="stable")]            # any order
+        tr = T._one("p99", np.zeros(n, np.int32), np.ones(n, np.int32), o, np.zeros(n, np.uint8), 10 ** 9, 1, 1)
+        r = oracle.simulate(tr, oracle.FCFS)
+        assert int(r.total_latency[0]) == n * (n + 1) // 2
+        assert int(r.p99_latency[0]) == want, n
 
 
 # ---------------------------------------------------------------------------------------------
