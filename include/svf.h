@@ -16,8 +16,16 @@
  *
  * Conventions for every entry point
  *  - DEVICE pointers are marked [dev]; HOST pointers [host].  The caller owns every buffer; the
- *    library allocates nothing and keeps no global state.  Scratch comes from the caller (`ws`,
- *    [dev], 256-byte aligned, size from the matching *_workspace_bytes call).
+ *    library allocates no device memory and the compute calls keep no state between calls: they
+ *    are re-entrant and may run concurrently on different streams (each with its own `ws`).  The
+ *    only state the library holds is per HOST THREAD and belongs to the measurement aids at the
+ *    end of this header (launch counters, the profiling switch and its CUDA events).
+ *  - Scratch comes from the caller: `ws` [dev], at least the bytes the matching *_workspace_bytes
+ *    call returns (that figure includes the slack for aligning `ws` up to 256 bytes).  A NULL or
+ *    short `ws` is SVF_EWORKSPACE, found on the host before anything touches the device.
+ *  - An array that would only be read for requests that do not exist may be NULL: with n = 0
+ *    (n_wait = 0, n_requests = 0) every per-request pointer may be NULL, `bit` included, also
+ *    under SVF_SVF_1BIT (O0, O1 >= 1 are still required there).
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls only
  *    enqueue work; outputs are valid once the stream has been synchronised.
  *  - Return value: svf_status_t for errors the HOST can see (arguments, sizes, CUDA launch
@@ -42,7 +50,10 @@ typedef enum { SVF_SVF = 0, SVF_SVF_1BIT = 1, SVF_SJF = 2, SVF_FCFS = 3 } svf_po
 
 typedef enum {
     SVF_OK = 0,
-    SVF_EINVAL = 1,       /* host: null pointer, negative size, unknown policy, O0/O1 < 1, missing bit */
+    SVF_EINVAL = 1,       /* host: null pointer, negative size, unknown policy, O0/O1 < 1, missing bit;
+                             data (svf_simulate, svf_volume_lower_bound): `offsets` not non-decreasing
+                             from 0 to N, or an instance larger than max_instance -- then every
+                             instance of the call reports it and nothing is simulated              */
     SVF_EWORKSPACE = 2,   /* host: ws is NULL or ws_bytes too small                                   */
     SVF_ECUDA = 3,        /* host: no device / launch failed (cudaGetLastError != success)           */
     SVF_ERANGE = 16,      /* data: o_i < 1, s_i < 0, a_i < 0 or output_key_i < 1 (running set: rem < 1 or kv < 0) */
@@ -149,7 +160,8 @@ int svf_simulate_policies(const svf_trace_t* trace, int n_policies, const int* p
  * lb_out[j]; TEL(policy) * M / lb_out[j] upper-bounds the policy's approximation ratio where the
  * optimum cannot be computed.  Arrivals, `bit` and `output_key` are not read.  lb_out: [dev] [I]
  * int64; status_out: [dev] [I] int32 or NULL: SVF_OK, SVF_ERANGE (o_i < 1 or s_i < 0),
- * SVF_EOVERFLOW (bound >= 2^63), SVF_EINVAL (bad offsets); lb_out[j] = 0 unless SVF_OK.
+ * SVF_EOVERFLOW (some volume >= 2^32 -- the width rule of every key, R11 -- or bound >= 2^63),
+ * SVF_EINVAL (bad offsets); lb_out[j] = 0 unless SVF_OK.
  * Keys + the same presort as svf_simulate + one reduction kernel. */
 size_t svf_volume_lower_bound_workspace_bytes(const svf_trace_t* trace);
 int svf_volume_lower_bound(const svf_trace_t* trace, int64_t* lb_out, int32_t* status_out, void* ws,

@@ -151,6 +151,13 @@ def _stream(stream):
     return C.c_void_p(s.cuda_stream)
 
 
+def _hold(ws: torch.Tensor, stream) -> None:
+    """A workspace allocated inside a call is dropped when the call returns while its kernels are only
+    enqueued: tell the caching allocator which stream still uses it (same-stream reuse is ordered)."""
+    if stream is not None and stream != torch.cuda.current_stream(ws.device):
+        ws.record_stream(stream)
+
+
 def _check(rc: int, where: str):
     if rc != OK:
         raise SvfError(rc, where)
@@ -190,6 +197,7 @@ def svf_sort_words(words, bit_lo=0, bit_hi=64, out=None, ws=None, stream=None):
                               int(bit_lo), int(bit_hi), C.c_void_p(ws.data_ptr()), ws.numel(),
                               _stream(stream))
     _check(rc, "svf_sort_words")
+    _hold(ws, stream)
     return out
 
 
@@ -230,6 +238,8 @@ def svf_admit(policy, M, t, w_s, w_o, w_a, w_bit, O0, O1, r_kv, r_rem, want_sort
                          _ptr(out.status, torch.int32, "status"), C.c_void_p(ws.data_ptr()),
                          ws.numel(), _stream(stream))
     _check(rc, "svf_admit")
+    _hold(ws, stream)
+    out._ws = ws  # keep the scratch alive until the caller drops the result
     return out
 
 
@@ -338,6 +348,7 @@ def svf_simulate(dt: DeviceTrace, policy: int, M: Optional[int] = None, out: Opt
     rc = lib().svf_simulate(C.byref(tr), int(policy), M, C.byref(res), C.c_void_p(ws.data_ptr()),
                             ws.numel(), _stream(stream))
     _check(rc, "svf_simulate")
+    _hold(ws, stream)
     out._ws = ws  # keep the scratch alive until the caller drops the result
     return out
 
@@ -366,6 +377,7 @@ def svf_simulate_policies(dt: DeviceTrace, policies, M: Optional[int] = None, ou
     rc = lib().svf_simulate_policies(C.byref(tr), len(policies), pol, M, res, C.c_void_p(ws.data_ptr()),
                                      ws.numel(), _stream(stream))
     _check(rc, "svf_simulate_policies")
+    _hold(ws, stream)
     for o in outs:
         o._ws = ws
     return outs
@@ -385,4 +397,5 @@ def svf_volume_lower_bound(dt: DeviceTrace, ws: Optional[torch.Tensor] = None, s
     rc = lib().svf_volume_lower_bound(C.byref(tr), C.c_void_p(lb.data_ptr()), C.c_void_p(st.data_ptr()),
                                       C.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream))
     _check(rc, "svf_volume_lower_bound")
+    _hold(ws, stream)
     return lb[: dt.n_instances], st[: dt.n_instances]

@@ -2,6 +2,15 @@
 // forward-looking check; P:L926 maxima at completion times).
 //   keys (svf_keys.cu) -> onesweep sort of the packed words on the key bits [32, 64)
 //   running set: words (2^32-1-rem, index) sorted the same way -> latest finish first
+//   k_admit_prefix (the usual path): feasibility is MONOTONE in the candidate set (adding a request
+//   adds a positive amount at every time it is alive), so the greedy loop's answer is the maximal
+//   feasible prefix of the priority order.  One CTA takes the running set and the
+//   first K_c candidates (K_c = min(n_wait, 8192 - n_run)), sorts them together by remaining steps
+//   (descending; stable radix passes in shared memory), keeps each thread's eight consecutive
+//   entries in registers and BISECTS the prefix length m: one check = the completion-time form of
+//   the forward-looking test on running + {candidates of rank < m} = a masked block scan of
+//   (kv, count) + max, about a microsecond; 14 checks instead of thousands of serial admissions.
+//   Only if all K_c candidates fit and more are waiting (or n_run > 4096) the serial path runs:
 //   k_admit: one CTA builds (f_j, A_j) in finish order with a block scan (svf_state.cuh) and checks
 //   the running set; then k_admit_slots (M < 2^30) takes the set into REGISTER SLOTS and pops the
 //   sorted queue with the fused evaluation pass of svf_sim_slots.cuh while the check passes;
@@ -11,6 +20,7 @@
 #include "svf_internal.cuh"
 #include "svf_state.cuh"
 #include "svf_sim_slots.cuh"
+#include "svf_segsort.cuh"
 
 namespace svf {
 
@@ -69,6 +79,174 @@ __device__ __forceinline__ int64_t block_incl_scan_i64(int64_t v, int64_t* warp_
     return v + off;
 }
 
+// ---- the maximal feasible prefix by bisection (a4 + a5), one CTA -------------------------------
+constexpr int AP_THREADS = 1024;
+constexpr int AP_IPT = 8;
+constexpr int AP_CAP = AP_THREADS * AP_IPT;          // running + candidate entries held on chip
+constexpr int AP_RUN_MAX = AP_CAP / 2;               // larger running sets take the serial path
+constexpr size_t AP_SMEM = (size_t)2 * AP_CAP * 8 + (size_t)AP_CAP * 4 + (size_t)(AP_THREADS / 32) * SORT_RADIX * 4;
+
+// fast[0] = 1: this kernel has answered (outputs written); 0: the serial kernels must run, and
+// rsorted_out holds the running set in their order (latest finish first, ties in input order).
+__global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64_t n_wait, const int32_t* __restrict__ w_s,
+                                                                const int32_t* __restrict__ w_o, int n_run,
+                                                                const int32_t* __restrict__ r_kv,
+                                                                const int32_t* __restrict__ r_rem,
+                                                                const SortPlan* __restrict__ wplan,
+                                                                const AdmitFlags* __restrict__ fl,
+                                                                uint64_t* __restrict__ rsorted_out, int* __restrict__ fast,
+                                                                int64_t* __restrict__ n_admitted_out,
+                                                                int32_t* __restrict__ admitted_idx_out,
+                                                                int32_t* __restrict__ status_out)
+{
+    constexpr int WARPS = AP_THREADS / 32;
+    extern __shared__ __align__(16) char ap_smem[];
+    uint64_t* buf0 = reinterpret_cast<uint64_t*>(ap_smem);
+    uint64_t* buf1 = buf0 + AP_CAP;
+    int32_t* kv_e = reinterpret_cast<int32_t*>(buf1 + AP_CAP);          // kv by entry id
+    uint32_t* whist = reinterpret_cast<uint32_t*>(kv_e + AP_CAP);
+    __shared__ uint32_t toff_s[SORT_RADIX];
+    __shared__ uint32_t warp_tot[WARPS];
+    __shared__ int64_t wsum_s[WARPS];
+    __shared__ int wcnt_s[WARPS];
+    __shared__ int red_s[2];
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+
+    int32_t status = SVF_OK;
+    if (fl->first_bad != ~0ull) status = (fl->first_bad & 1ull) ? SVF_EUNSORTED : SVF_ERANGE;
+    else if (fl->run_bad) status = SVF_ERANGE;
+    else if (fl->key_status != SVF_OK) status = fl->key_status;
+    if (status != SVF_OK) {
+        if (tid == 0) { *n_admitted_out = 0; if (status_out) *status_out = status; *fast = 1; }
+        return;
+    }
+
+    // entries: e < R the running set as given (kv, rem); e >= R the candidate of priority rank e - R,
+    // started now: it holds s now and has o steps left
+    const uint64_t* __restrict__ wsorted = wplan->result;
+    const int R = n_run;
+    const int Kc = (int)(n_wait < (int64_t)(AP_CAP - R) ? n_wait : (int64_t)(AP_CAP - R));
+    const int E = R + Kc;
+    int rem_l[AP_IPT];
+    int maxrem = 0;
+#pragma unroll
+    for (int i = 0; i < AP_IPT; ++i) {
+        const int e = tid + i * AP_THREADS;
+        rem_l[i] = 0;
+        if (e < R) { kv_e[e] = r_kv[e]; rem_l[i] = r_rem[e]; }
+        else if (e < E) { const uint32_t h = (uint32_t)wsorted[e - R]; kv_e[e] = w_s[h]; rem_l[i] = w_o[h]; }
+        maxrem = rem_l[i] > maxrem ? rem_l[i] : maxrem;
+    }
+    maxrem = __reduce_max_sync(FULL, maxrem);
+    if (tid < 2) red_s[tid] = 0;
+    __syncthreads();
+    if (lane == 0) atomicMax(&red_s[0], maxrem);
+    __syncthreads();
+    maxrem = red_s[0];
+    // word = (maxrem - rem) << 32 | e: ascending = latest finish first, equal rem in entry order
+    uint32_t kor = 0;
+#pragma unroll
+    for (int i = 0; i < AP_IPT; ++i) {
+        const int e = tid + i * AP_THREADS;
+        if (e < E) {
+            const uint32_t key = (uint32_t)(maxrem - rem_l[i]);
+            buf0[e] = ((uint64_t)key << 32) | (uint32_t)e;
+            kor |= key;
+        }
+    }
+    kor = __reduce_or_sync(FULL, kor);
+    if (lane == 0 && kor) atomicOr(reinterpret_cast<unsigned int*>(&red_s[1]), kor);
+    __syncthreads();
+    const uint32_t kall = (uint32_t)red_s[1];
+    const int npass = ((kall ? 32 - __clz(kall) : 0) + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
+    const int ipt = (E + AP_THREADS - 1) / AP_THREADS;
+    for (int p = 0; p < npass; ++p) {
+        seg_pass<AP_THREADS, AP_IPT>(buf0, buf1, E, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
+        uint64_t* tmp = buf0; buf0 = buf1; buf1 = tmp;
+    }
+    __syncthreads();
+
+    // this thread's eight consecutive entries of the completion-time order, in registers
+    int kv[AP_IPT], rem[AP_IPT], rk[AP_IPT];          // rk: priority rank, -1 = running (always in the set)
+#pragma unroll
+    for (int i = 0; i < AP_IPT; ++i) {
+        const int p = tid * AP_IPT + i;
+        kv[i] = 0; rem[i] = 0; rk[i] = INT_MAX;       // past the end: never in the set
+        if (p < E) {
+            const uint64_t w = buf0[p];
+            const int e = (int)(uint32_t)w;
+            rem[i] = maxrem - (int)(uint32_t)(w >> 32);
+            kv[i] = kv_e[e];
+            rk[i] = e < R ? -1 : e - R;
+        }
+    }
+
+    // feasible(m): with S_m = running + {candidates of rank < m} in this order, every entry of S_m
+    // has  sum_{earlier or same, in S_m} kv + rem * #{earlier or same, in S_m}  <= M   (an
+    // entry inside a group of equal rem sees a partial sum, which is below the group's last entry)
+    auto feasible = [&](int m) -> bool {
+        int64_t s = 0; int c = 0;
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) if (rk[i] < m) { s += kv[i]; ++c; }
+        int64_t si = s; int ci = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int64_t x = __shfl_up_sync(FULL, si, d); const int y = __shfl_up_sync(FULL, ci, d);
+            if (lane >= d) { si += x; ci += y; }
+        }
+        if (lane == 31) { wsum_s[wrp] = si; wcnt_s[wrp] = ci; }
+        __syncthreads();
+        int64_t ws = wsum_s[lane]; int wc = wcnt_s[lane];       // WARPS == 32: one warp total per lane
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int64_t x = __shfl_up_sync(FULL, ws, d); const int y = __shfl_up_sync(FULL, wc, d);
+            if (lane >= d) { ws += x; wc += y; }
+        }
+        int64_t pre = si - s + (wrp > 0 ? __shfl_sync(FULL, ws, wrp - 1) : 0);
+        int cnt = ci - c + (wrp > 0 ? __shfl_sync(FULL, wc, wrp - 1) : 0);
+        bool bad = false;
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i)
+            if (rk[i] < m) { pre += kv[i]; ++cnt; bad |= pre + (int64_t)rem[i] * cnt > M; }
+        return __syncthreads_or(bad) == 0;               // also fences wsum_s / wcnt_s for the next call
+    };
+    static_assert(WARPS == 32, "the second scan level holds one warp total per lane");
+
+    int lo = 0, hi = Kc + 1;                                 // feasible(lo) (or nobody fits at all), !feasible(hi)
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (feasible(mid)) lo = mid; else hi = mid;
+    }
+    if (lo == Kc && (int64_t)Kc < n_wait) {
+        // every candidate held here fits and more are waiting: the serial kernels take over; give
+        // them the running set in finish order (its entries, compacted from the order above)
+        int c = 0;
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) c += rk[i] == -1;
+        int ci = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(FULL, ci, d); if (lane >= d) ci += y; }
+        if (lane == 31) wcnt_s[wrp] = ci;
+        __syncthreads();
+        int wc = wcnt_s[lane];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(FULL, wc, d); if (lane >= d) wc += y; }
+        int q = ci - c + (wrp > 0 ? __shfl_sync(FULL, wc, wrp - 1) : 0);
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) {
+            if (rk[i] == -1) {
+                const uint32_t e = (uint32_t)buf0[tid * AP_IPT + i];
+                rsorted_out[q++] = ((uint64_t)(0xffffffffu - (uint32_t)rem[i]) << 32) | e;
+            }
+        }
+        if (tid == 0) *fast = 0;
+        return;
+    }
+    if (admitted_idx_out)
+        for (int k = tid; k < lo; k += AP_THREADS) admitted_idx_out[k] = (int32_t)(uint32_t)wsorted[k];
+    if (tid == 0) { *n_admitted_out = lo; if (status_out) *status_out = SVF_OK; *fast = 1; }
+}
+
 __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, int64_t n_wait,
                                                          const int32_t* __restrict__ w_s,
                                                          const int32_t* __restrict__ w_o,
@@ -76,6 +254,8 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
                                                          const int32_t* __restrict__ r_rem,
                                                          const SortPlan* __restrict__ wplan,
                                                          const SortPlan* __restrict__ rplan,
+                                                         const uint64_t* __restrict__ rsorted_direct /* or NULL: rplan */,
+                                                         const int* __restrict__ fast /* or NULL */,
                                                          const AdmitFlags* __restrict__ fl,
                                                          int32_t* __restrict__ f, int64_t* __restrict__ A,
                                                          int64_t* __restrict__ n_admitted_out,
@@ -86,6 +266,7 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
     __shared__ int scratch[2][64];
     __shared__ int64_t warp_tot[ADMIT_THREADS / 32];
     if (handoff && threadIdx.x == 0) *handoff = 0;
+    if (fast && *fast) return;                 // k_admit_prefix has answered
     int parity = 0;
     const int tid = threadIdx.x;
 
@@ -100,7 +281,7 @@ __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, i
 
     // running set, latest finish first: f_j = rem_j (time is counted from now), A_j = sum_{i<=j}
     // kv_i + rem_j (j+1) = mem at its completion
-    const uint64_t* __restrict__ rsorted = rplan->result;
+    const uint64_t* __restrict__ rsorted = rsorted_direct ? rsorted_direct : rplan->result;
     int64_t carry = 0;
     uint32_t bad = 0;
     for (int64_t c = 0; c < n_run; c += ADMIT_THREADS) {
@@ -150,6 +331,7 @@ __global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wa
                                                          const int32_t* __restrict__ r_kv,
                                                          const SortPlan* __restrict__ wplan,
                                                          const SortPlan* __restrict__ rplan,
+                                                         const uint64_t* __restrict__ rsorted_direct /* or NULL: rplan */,
                                                          const int* __restrict__ handoff,
                                                          const int32_t* __restrict__ f_arr, const int64_t* __restrict__ A_arr,
                                                          int32_t* __restrict__ ef, uint32_t* __restrict__ eB,
@@ -168,7 +350,7 @@ __global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wa
     if (*handoff == 0) return;               // data error or infeasible running set: k_admit has answered
     const int tid = threadIdx.x;
     const int Mi = (int)M;
-    const uint64_t* __restrict__ rsorted = rplan->result;
+    const uint64_t* __restrict__ rsorted = rsorted_direct ? rsorted_direct : rplan->result;
     const uint64_t* __restrict__ wsorted = wplan->result;
     const int R = (int)n_run;
     int f[K]; uint32_t B[K], c[K];
@@ -241,6 +423,7 @@ struct AdmitWs {
     int32_t* f; int64_t* A;
     int32_t* ef; uint32_t *eB, *ec;   // ext slots of the register-slot kernel
     int* handoff;
+    int* fast;              // written by k_admit_prefix: 1 = answered, 0 = the serial kernels run
     AdmitFlags* flags;
     size_t total;
 };
@@ -263,7 +446,7 @@ void admit_ws_layout(AdmitWs* w, char* base, int64_t n_wait, int64_t n_run)
     w->ef = (int32_t*)(base + p); p += align_up(cap * 4, 256);
     w->eB = (uint32_t*)(base + p); p += align_up(cap * 4, 256);
     w->ec = (uint32_t*)(base + p); p += align_up(cap * 4, 256);
-    w->handoff = (int*)(base + p); p += 256;
+    w->handoff = (int*)(base + p); w->fast = w->handoff + 1; p += 256;
     w->flags = (AdmitFlags*)(base + p); p += 256;
     w->total = p;
 }
@@ -300,13 +483,12 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     if (n_wait > 0 && (!w_s || !w_o || !w_a)) return SVF_EINVAL;
     if (n_run > 0 && (!r_kv || !r_rem)) return SVF_EINVAL;
     if (!ws) return SVF_EWORKSPACE;
-    int dev_count = 0;
-    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
     char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
-    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
     AdmitWs w;
     admit_ws_layout(&w, base, n_wait, n_run);
-    if (w.total > avail) return SVF_EWORKSPACE;
+    if ((size_t)(base - (char*)ws) + w.total > ws_bytes) return SVF_EWORKSPACE;
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
     cudaStream_t st = (cudaStream_t)stream;
 
     k_admit_init<<<1, 1, 0, st>>>(w.flags);
@@ -325,16 +507,27 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     // a3: the waiting queue in priority order; the running set by finish time
     rc = sort_u64(w.wsort, w.w0, w.w1, w.w0, n_wait, 32, 64, st, &g_launches_admit);
     if (rc) return SVF_ECUDA;
-    rc = sort_u64(w.rsort, w.r0, w.r1, w.r0, n_run, 32, 64, st, &g_launches_admit);
-    if (rc) return SVF_ECUDA;
-    // a4 + a5
+    // a4 + a5: the maximal feasible prefix by bisection on one CTA; it also orders the running set
+    // (for the serial kernels, should they be needed), so the device-wide sort of it is skipped
+    const bool prefix = n_run <= AP_RUN_MAX;
+    if (prefix) {
+        if (cudaFuncSetAttribute(k_admit_prefix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
+        k_admit_prefix<<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
+                                                       w.fast, n_admitted_out, admitted_idx_out, status_out);
+        ++g_launches_admit;
+    } else {
+        rc = sort_u64(w.rsort, w.r0, w.r1, w.r0, n_run, 32, 64, st, &g_launches_admit);
+        if (rc) return SVF_ECUDA;
+    }
+    const uint64_t* rdirect = prefix ? w.r1 : nullptr;
+    const int* fast = prefix ? w.fast : nullptr;
     const bool slots = M < ((int64_t)1 << 30);        // 32-bit wrapping arithmetic of the slot passes is exact
-    k_admit<<<1, ADMIT_THREADS, 0, st>>>(M, t, n_wait, w_s, w_o, n_run, r_kv, r_rem, w.wsort.plan, w.rsort.plan,
+    k_admit<<<1, ADMIT_THREADS, 0, st>>>(M, t, n_wait, w_s, w_o, n_run, r_kv, r_rem, w.wsort.plan, w.rsort.plan, rdirect, fast,
                                          w.flags, w.f, w.A, n_admitted_out, admitted_idx_out, status_out,
                                          slots ? w.handoff : nullptr);
     ++g_launches_admit;
     if (slots) {
-        k_admit_slots<256><<<1, 256, 0, st>>>(M, n_wait, w_s, w_o, n_run, r_kv, w.wsort.plan, w.rsort.plan, w.handoff,
+        k_admit_slots<256><<<1, 256, 0, st>>>(M, n_wait, w_s, w_o, n_run, r_kv, w.wsort.plan, w.rsort.plan, rdirect, w.handoff,
                                               w.f, w.A, w.ef, w.eB, w.ec, n_admitted_out, admitted_idx_out, status_out);
         ++g_launches_admit;
     }

@@ -51,10 +51,10 @@ extern "C" int svf_sort_words(int64_t n, const uint64_t* words_in, uint64_t* wor
     if (n < 0 || n >= ((int64_t)1 << 30) || bit_lo < 0 || bit_hi > 64 || bit_lo >= bit_hi) return SVF_EINVAL;
     if (n > 0 && (!words_in || !words_out || words_in == words_out)) return SVF_EINVAL;
     if (!ws) return SVF_EWORKSPACE;
-    if (!have_device()) return SVF_ECUDA;
     char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
     const size_t need = svf_sort_workspace_bytes(n, bit_lo, bit_hi) - 256;
     if ((size_t)(base - (char*)ws) + need > ws_bytes) return SVF_EWORKSPACE;
+    if (!have_device()) return SVF_ECUDA;
     SortWs w;
     sort_ws_carve(&w, base, n, bit_lo, bit_hi);
     uint64_t* tmp = (uint64_t*)(base + align_up(sort_ws_bytes(n, bit_lo, bit_hi), 256));

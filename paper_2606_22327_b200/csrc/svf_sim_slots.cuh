@@ -142,6 +142,7 @@ struct SlotArgs {
     int n_policies;
     PolicyIO io[MAX_POLICIES];
     unsigned long long* work_ctr;
+    const uint32_t* layout_bad;      // one word: the offsets of the call are not monotone (k_sim_check_layout)
     unsigned long long* work_counts; // [4] E, U, evaluations, blocked evaluations (COUNT variant only)
     char* gstate; size_t slot_bytes; // per-CTA state when it does not fit in shared memory
     int ecap;                        // ext slots per instance
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
         const int64_t n64 = g.off[j + 1] - base;
         uint32_t flags = 0;
         if (n64 < 0 || n64 > g.max_instance || base < 0 || base + (n64 > 0 ? n64 : 0) > g.N ||
-            g.off[0] != 0 || g.off[g.I] != g.N || (QREG && n64 > QREG_RANKS))
+            g.off[0] != 0 || g.off[g.I] != g.N || (QREG && n64 > QREG_RANKS) || *g.layout_bad)
             flags |= F_LAYOUT;
         const int n = (flags & F_LAYOUT) ? 0 : (int)n64;
         const int32_t* __restrict__ a = g.a + base;
@@ -619,6 +620,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                     rounds += (uint32_t)(tn - t - 1);
                     decisions += (uint32_t)(tn - t - 1);
                 }
+                if (tn == INT_MAX) break;                     // nothing left that could ever happen (corrupt rank[]): never spin
                 t = tn;
             }
             flush(started & 31);

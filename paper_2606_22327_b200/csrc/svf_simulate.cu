@@ -43,6 +43,7 @@ struct SimArgs {
     int32_t *makespan, *status;
     uint64_t* latw;                  // [N] (instance << 32) + latency, or NULL
     unsigned long long* work_ctr;
+    const uint32_t* layout_bad;      // one word: the offsets of the call are not monotone (k_sim_check_layout)
     char* gstate;                    // per-CTA state slots when the state is not in shared memory
     size_t slot_bytes;
     int cap;                         // entries per state slot
@@ -53,6 +54,21 @@ __host__ __device__ inline size_t state_bytes(int cap)
     int nL0 = (cap + 31) / 32, nL1 = (nL0 + 31) / 32;
     return align_up((size_t)cap * 8, 16) + align_up((size_t)cap * 4, 16) + align_up((size_t)nL0 * 4, 16) +
            align_up((size_t)nL1 * 4, 16);
+}
+
+// The offsets of a call must be non-decreasing from 0 to N: otherwise two instances that each look
+// valid could overlap and their presorts would race on order[] / rank[].  One flag word for the
+// whole call; when it is set every instance reports SVF_EINVAL and nothing is simulated.
+__global__ void __launch_bounds__(256) k_sim_check_layout(int64_t I, int64_t N, const int64_t* __restrict__ off,
+                                                          uint32_t* __restrict__ layout_bad)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < I; j += stride) {
+        const int64_t lo = off[j], hi = off[j + 1];
+        if (lo > hi || lo < 0 || hi > N || (j == 0 && lo != 0) || (j == I - 1 && hi != N)) bad = true;
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(layout_bad, 1u);
 }
 
 // ---- Phase A ---------------------------------------------------------------------------------
@@ -126,7 +142,7 @@ __global__ void __launch_bounds__(THREADS) k_sim(SimArgs g)
         const int64_t n64 = g.off[j + 1] - base;
         uint32_t flags = 0;
         if (n64 < 0 || n64 > g.max_instance || base < 0 || base + (n64 > 0 ? n64 : 0) > g.N ||
-            g.off[0] != 0 || g.off[g.I] != g.N)
+            g.off[0] != 0 || g.off[g.I] != g.N || *g.layout_bad)
             flags |= F_LAYOUT;
         const int n = (flags & F_LAYOUT) ? 0 : (int)n64;
         const int32_t* __restrict__ a = g.a + base;
@@ -286,6 +302,7 @@ __global__ void k_sim_p99(int64_t I, const int64_t* __restrict__ off, const Sort
 __global__ void __launch_bounds__(256) k_volume_lb(int64_t I, int64_t N, int64_t max_instance,
                                                    const int64_t* __restrict__ off, const int32_t* __restrict__ s,
                                                    const int32_t* __restrict__ o, const uint32_t* __restrict__ order,
+                                                   const uint32_t* __restrict__ layout_bad,
                                                    int64_t* __restrict__ lb_out, int32_t* __restrict__ status_out)
 {
     __shared__ unsigned long long part[8][2];
@@ -294,7 +311,7 @@ __global__ void __launch_bounds__(256) k_volume_lb(int64_t I, int64_t N, int64_t
     for (int64_t j = blockIdx.x; j < I; j += gridDim.x) {
         const int64_t base = off[j], n = off[j + 1] - base;
         uint32_t flags = 0;
-        if (n < 0 || n > max_instance || base < 0 || base + (n > 0 ? n : 0) > N || off[0] != 0 || off[I] != N) flags |= F_LAYOUT;
+        if (n < 0 || n > max_instance || base < 0 || base + (n > 0 ? n : 0) > N || off[0] != 0 || off[I] != N || *layout_bad) flags |= F_LAYOUT;
         if (tid == 0) flags_s = 0;
         __syncthreads();
         unsigned __int128 acc = 0;
@@ -303,7 +320,9 @@ __global__ void __launch_bounds__(256) k_volume_lb(int64_t I, int64_t N, int64_t
                 const int64_t i = base + order[base + r];
                 const int32_t si = s[i], oi = o[i];
                 if (oi < 1 || si < 0) flags |= F_RANGE;
-                acc += (unsigned __int128)priority_key(SVF_SVF, si, oi, 0, 0u, 0, 0) * (unsigned long long)(n - r);
+                const uint64_t vol = priority_key(SVF_SVF, si, oi, 0, 0u, 0, 0);
+                if (oi >= 1 && si >= 0 && (vol >> 32)) flags |= F_OVERFLOW;   // the presort orders 32-bit keys (R11)
+                acc += (unsigned __int128)vol * (unsigned long long)(n - r);
             }
         }
 #pragma unroll
@@ -336,8 +355,9 @@ struct SimWs {
     int4* req[MAX_POLICIES];          // [N] each
     uint32_t* lat[MAX_POLICIES];      // [N] each: latencies for the in-kernel p99 selection
     int32_t* status_tmp[MAX_POLICIES];// [I] each, when the caller does not want status
-    unsigned long long* counts;   // [2] E, U of the counting variant
+    unsigned long long* counts;   // [4] E, U, evaluations, blocked evaluations of the counting variant
     unsigned long long* work_ctr;
+    uint32_t* layout_bad;         // one word, 8 bytes behind work_ctr (zeroed with it)
     char* gstate;
     size_t slot_bytes;
     int grid_slots;
@@ -505,7 +525,8 @@ void sim_ws_layout(SimWs* w, char* base, const svf_trace_t* tr, const SimConfig&
         w->status_tmp[q] = (int32_t*)(base + p); p += align_up((size_t)(I > 0 ? I : 1) * 4, 256);
     }
     w->counts = (unsigned long long*)(base + p); p += 256;
-    w->work_ctr = (unsigned long long*)(base + p); p += 256;
+    w->work_ctr = (unsigned long long*)(base + p);
+    w->layout_bad = (uint32_t*)(base + p + 8); p += 256;
     w->slot_bytes = c.gslot_bytes;
     w->grid_slots = grid_slots;
     w->gstate = base + p; p += w->slot_bytes * (size_t)grid_slots;
@@ -568,7 +589,7 @@ int simulate_wide(const svf_trace_t* tr, int policy, int64_t M, const svf_result
     g.rounds = out->rounds; g.decisions = out->decisions; g.makespan = out->makespan;
     g.status = out->status ? out->status : w.status_tmp[0];
     g.latw = out->p99_latency ? w.words0 : nullptr;
-    g.work_ctr = w.work_ctr; g.gstate = w.gstate; g.slot_bytes = w.slot_bytes; g.cap = c.cap;
+    g.work_ctr = w.work_ctr; g.layout_bad = w.layout_bad; g.gstate = w.gstate; g.slot_bytes = w.slot_bytes; g.cap = c.cap;
     if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
     if (N > 0) {
         int64_t blocks = ceil_div(N, 256);
@@ -626,20 +647,31 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;          // packed sort word would not fit
     if (!ws) return SVF_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
+    // the caller's buffer must hold what the matching *_workspace_bytes call asks for (less its 256
+    // bytes of alignment slack) behind the alignment pad: checked before anything touches the device
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    if ((size_t)(base - (char*)ws) + (sim_workspace_bytes(tr, P) - 256) > ws_bytes) return SVF_EWORKSPACE;
 
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
 
-    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
-    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
     int grid = sim_grid_any(c, I * P);
     if (c.gslot_bytes && grid > c.max_cta_per_sm * sm_count()) grid = c.max_cta_per_sm * sm_count();
     SimWs w;
     sim_ws_layout(&w, base, tr, c, c.gslot_bytes ? grid : 0, P);
-    if (w.total > avail) return SVF_EWORKSPACE;
+    if ((size_t)(base - (char*)ws) + w.total > ws_bytes) return SVF_EWORKSPACE;
 
     g_events_valid = false;
     prof_mark(0, st);
+    // the call-wide layout flag (zeroed here; the per-policy work counter is zeroed again below)
+    if (cudaMemsetAsync(w.work_ctr, 0, 16, st) != cudaSuccess) return SVF_ECUDA;
+    {
+        int64_t blocks = ceil_div(I, 256);
+        const int64_t capb = (int64_t)sm_count() * 4;
+        if (blocks > capb) blocks = capb;
+        k_sim_check_layout<<<(unsigned)blocks, 256, 0, st>>>(I, N, tr->offsets, w.layout_bad);
+        ++g_launches_sim;
+    }
     if (!c.slots) {
         // M >= 2^30: the wide kernel, one policy after the other
         int rc = SVF_OK;
@@ -654,7 +686,6 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     q.O0 = tr->O0; q.O1 = tr->O1;
     q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.okey = tr->output_key; q.bit = tr->bit;
     q.n_policies = P;
-    if (cudaMemsetAsync(w.work_ctr, 0, sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
     for (int k = 0; k < P; ++k) {
         const svf_result_t* out = &outs[k];
         PolicyIO& io = q.io[k];
@@ -690,7 +721,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     prof_mark(1, st);
 
     // ---- phase B: one persistent launch over P x I work items -------------------------------------
-    q.work_ctr = w.work_ctr; q.work_counts = w.counts;
+    q.work_ctr = w.work_ctr; q.work_counts = w.counts; q.layout_bad = w.layout_bad;
     q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
     const bool count = g_profiling == 2;
     if (count) {
@@ -763,14 +794,21 @@ extern "C" int svf_volume_lower_bound(const svf_trace_t* tr, int64_t* lb_out, in
     SimConfig c = sim_config(tr, 0, 1);
     if (c.sb + 32 + c.ib > 64) return SVF_EINVAL;
     if (!ws) return SVF_EWORKSPACE;
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    if ((size_t)(base - (char*)ws) + (sim_workspace_bytes(tr, 1) - 256) > ws_bytes) return SVF_EWORKSPACE;
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
     cudaStream_t st = (cudaStream_t)stream;
-    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
-    const size_t avail = ws_bytes - (size_t)(base - (char*)ws);
     SimWs w;
     sim_ws_layout(&w, base, tr, c, 0, 1);
-    if (w.total - w.slot_bytes * (size_t)w.grid_slots > avail) return SVF_EWORKSPACE;
+    if (cudaMemsetAsync(w.work_ctr, 0, 16, st) != cudaSuccess) return SVF_ECUDA;
+    {
+        int64_t blocks = ceil_div(I, 256);
+        const int64_t capb = (int64_t)sm_count() * 4;
+        if (blocks > capb) blocks = capb;
+        k_sim_check_layout<<<(unsigned)blocks, 256, 0, st>>>(I, N, tr->offsets, w.layout_bad);
+        ++g_launches_sim;
+    }
     // volumes ascending = the SVF order under the TRUE lengths (no predicted keys here)
     if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
         if (seg_sort_keys(SVF_SVF, I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, nullptr,
@@ -795,7 +833,7 @@ extern "C" int svf_volume_lower_bound(const svf_trace_t* tr, int64_t* lb_out, in
     int64_t grid = (int64_t)sm_count() * 8;
     if (grid > I) grid = I;
     k_volume_lb<<<(unsigned)grid, 256, 0, st>>>(I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, w.order[0],
-                                                lb_out, status_out);
+                                                w.layout_bad, lb_out, status_out);
     ++g_launches_sim;
     return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
 }

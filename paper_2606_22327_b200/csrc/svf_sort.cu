@@ -21,6 +21,7 @@
 //  * The plan kernel ping-pongs the two buffers so that the last EXECUTED pass lands in the
 //    caller's output buffer: no copy afterwards.
 #include "svf_internal.cuh"
+#include "svf_segsort.cuh"
 
 namespace svf {
 
@@ -338,65 +339,6 @@ __global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan-
 // rank[] (rank of id) and, if wanted, the (s, o, id, a) records in priority order.  HBM traffic:
 // 12-13 B read + 8 B (24 B with records) written per request, against 8 + 16 B per executed pass
 // of the device-wide sort.
-template <int THREADS, int IPT>
-__device__ __forceinline__ void seg_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out, int n, int ipt,
-                                         int shift, uint32_t* whist, uint32_t* toff_s, uint32_t* warp_tot)
-{
-    constexpr int WARPS = THREADS / 32;
-    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-    for (int i = tid; i < WARPS * SORT_RADIX; i += THREADS) whist[i] = 0;
-    __syncthreads();
-    const int wbase = wrp * 32 * ipt;
-    uint32_t* wh = whist + wrp * SORT_RADIX;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    uint64_t key[IPT];            // IPT >= ipt: sized by the template so small segments stay cheap in registers
-    uint32_t rank[IPT];
-#pragma unroll
-    for (int i = 0; i < IPT; ++i) {
-        if (i >= ipt) break;                                   // uniform
-        const int e = wbase + i * 32 + lane;
-        const bool valid = e < n;
-        key[i] = valid ? in[e] : 0ull;
-        const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & 0xffu) : SORT_RADIX;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);   // one segment per CTA: latency matters, not issue slots
-        const int leader = 31 - __clz(peers);
-        uint32_t base = 0;
-        if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
-        base = __shfl_sync(0xffffffffu, base, leader);
-        __syncwarp();
-        rank[i] = base + __popc(peers & lt_mask);
-    }
-    __syncthreads();
-    // digit d (threads 0..255): exclusive scan over warps, then over digits
-    uint32_t count = 0;
-    if (tid < SORT_RADIX) {
-        uint32_t run = 0;
-#pragma unroll
-        for (int w = 0; w < WARPS; ++w) { uint32_t c = whist[w * SORT_RADIX + tid]; whist[w * SORT_RADIX + tid] = run; run += c; }
-        count = run;
-    }
-    uint32_t inc = count;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-    if (lane == 31) warp_tot[wrp] = inc;
-    __syncthreads();
-    if (tid < SORT_RADIX) {
-        uint32_t off = 0;
-        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
-        toff_s[tid] = off + inc - count;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < IPT; ++i) {
-        if (i >= ipt) break;
-        if (wbase + i * 32 + lane < n) {
-            const uint32_t d = (uint32_t)(key[i] >> shift) & 0xffu;
-            out[toff_s[d] + wh[d] + rank[i]] = key[i];
-        }
-    }
-    __syncthreads();
-}
-
 template <int IPT>
 __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I, int64_t N, int cap,
                                                            const int64_t* __restrict__ off,
@@ -452,18 +394,16 @@ __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I
 
 }  // namespace
 
+// SMs of the CURRENT device, asked every time (an attribute query, no device work): nothing is
+// cached per process, so threads driving different devices each get their own count; 148 (B200)
+// when there is no device, so that the host-side size computations still work there.
 int sm_count()
 {
-    static int cached = 0;
-    if (cached == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            cached = v;
-        else
-            return 148;
-    }
-    return cached;
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+        return v;
+    return 148;
 }
 
 static size_t sort_status_bytes(int64_t n, int bit_lo, int bit_hi)

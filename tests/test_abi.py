@@ -108,3 +108,116 @@ def test_binding_refuses_cpu_tensors(svf_lib):
     s = torch.ones(4, dtype=torch.int32)
     with pytest.raises(TypeError):
         binding.svf_keys(binding.SVF, s, s)
+
+
+# ---------------------------------------------------------------------------------------------
+# workspace errors are found on the host, before the device is touched (include/svf.h conventions)
+# ---------------------------------------------------------------------------------------------
+def _sim_protos(L):
+    from paper_2606_22327_b200.binding import _Result, _Trace
+    L.svf_simulate.restype = C.c_int
+    L.svf_simulate.argtypes = [C.POINTER(_Trace), C.c_int, C.c_int64, C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+    L.svf_simulate_workspace_bytes.restype = C.c_size_t
+    L.svf_simulate_workspace_bytes.argtypes = [C.POINTER(_Trace)]
+    L.svf_volume_lower_bound.restype = C.c_int
+    L.svf_volume_lower_bound.argtypes = [C.POINTER(_Trace), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+    L.svf_volume_lower_bound_workspace_bytes.restype = C.c_size_t
+    L.svf_volume_lower_bound_workspace_bytes.argtypes = [C.POINTER(_Trace)]
+    L.svf_admit.restype = C.c_int
+    L.svf_admit.argtypes = [C.c_int, C.c_int64, C.c_int32, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32, C.c_int64] + \
+                           [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+    L.svf_admit_workspace_bytes.restype = C.c_size_t
+    L.svf_admit_workspace_bytes.argtypes = [C.c_int64, C.c_int64]
+    L.svf_sort_words.restype = C.c_int
+    L.svf_sort_words.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+    L.svf_sort_workspace_bytes.restype = C.c_size_t
+    L.svf_sort_workspace_bytes.argtypes = [C.c_int64, C.c_int, C.c_int]
+    return _Trace, _Result
+
+
+# stand-ins for device pointers: the calls below must fail on the host before reading any of them
+P0, P1, WS = 0x10000, 0x20000, 0x7000100
+
+
+def test_short_and_unaligned_workspace_is_eworkspace(svf_lib):
+    """SVF_EWORKSPACE from every call that takes `ws`: NULL, one byte short, and an UNALIGNED `ws`
+    whose ws_bytes is smaller than the alignment pad (the size check must not wrap around)."""
+    L = svf_lib
+    _Trace, _Result = _sim_protos(L)
+    EWS = 2
+    tr = _Trace(3, 300, 100, P0, P0, P0, P0, P0, 1, 1, None)
+    res = _Result()
+    need = L.svf_simulate_workspace_bytes(C.byref(tr))
+    assert need > 300 * 8
+    for ws, nbytes in ((None, need), (WS, need - 257), (WS, 0), (WS + 1, 3), (WS + 1, 254), (WS + 255, need - 300)):
+        assert L.svf_simulate(C.byref(tr), 0, 1000, C.byref(res), ws, nbytes, None) == EWS, (ws, nbytes)
+        assert L.svf_volume_lower_bound(C.byref(tr), P1, None, ws, nbytes, None) == EWS, (ws, nbytes)
+    need = L.svf_admit_workspace_bytes(500, 40)
+    for ws, nbytes in ((None, need), (WS, need - 257), (WS + 1, 3), (WS + 8, 200)):
+        rc = L.svf_admit(0, 1000, 0, 500, P0, P0, P0, None, 1, 1, 40, P0, P0, P1, None, None, None, ws, nbytes, None)
+        assert rc == EWS, (ws, nbytes)
+    need = L.svf_sort_workspace_bytes(5000, 0, 64)
+    for ws, nbytes in ((None, need), (WS, need - 257), (WS + 1, 3), (WS + 8, 200)):
+        assert L.svf_sort_words(5000, P0, P1, 0, 64, ws, nbytes, None) == EWS, (ws, nbytes)
+
+
+def test_onebit_without_requests_needs_no_bit_array(svf_lib):
+    """n = 0 under SVF_SVF_1BIT with bit = NULL is NOT an argument error (svf.h conventions; the oracle
+    takes the same call, tests/test_oracle_pins.py); O0, O1 >= 1 are still required."""
+    L = svf_lib
+    _Trace, _Result = _sim_protos(L)
+    L.svf_keys.restype = C.c_int
+    L.svf_keys.argtypes = [C.c_int, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32] + [C.c_void_p] * 3
+    assert L.svf_keys(1, 0, None, None, None, None, 2, 8, None, None, None) != 1
+    assert L.svf_keys(1, 0, None, None, None, None, 0, 8, None, None, None) == 1
+    rc = L.svf_admit(1, 1000, 0, 0, None, None, None, None, 2, 8, 0, None, None, P1, None, None, None, WS, 1 << 20, None)
+    assert rc != 1
+    tr = _Trace(2, 0, 0, P0, None, None, None, None, 2, 8, None)
+    assert L.svf_simulate(C.byref(tr), 1, 1000, C.byref(_Result()), WS, 1 << 20, None) != 1
+
+
+_NO_DEVICE_SCRIPT = r"""
+import ctypes as C, sys
+sys.path.insert(0, {root!r})
+from paper_2606_22327_b200.binding import _Result, _Trace
+L = C.CDLL({lib!r})
+P0, P1, WS, BIG = 0x10000, 0x20000, 0x7000100, 1 << 30
+L.svf_keys.restype = C.c_int
+L.svf_keys.argtypes = [C.c_int, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32] + [C.c_void_p] * 3
+L.svf_simulate.restype = C.c_int
+L.svf_simulate.argtypes = [C.POINTER(_Trace), C.c_int, C.c_int64, C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+L.svf_simulate_policies.restype = C.c_int
+L.svf_simulate_policies.argtypes = [C.POINTER(_Trace), C.c_int, C.POINTER(C.c_int), C.c_int64, C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+L.svf_volume_lower_bound.restype = C.c_int
+L.svf_volume_lower_bound.argtypes = [C.POINTER(_Trace), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+L.svf_admit.restype = C.c_int
+L.svf_admit.argtypes = [C.c_int, C.c_int64, C.c_int32, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+L.svf_sort_words.restype = C.c_int
+L.svf_sort_words.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+tr = _Trace(3, 300, 100, P0, P0, P0, P0, P0, 1, 1, None)
+res = _Result()
+pol = (C.c_int * 2)(0, 3)
+outs = (_Result * 2)()
+rcs = [L.svf_keys(0, 100, P0, P0, None, None, 1, 1, P1, None, None),
+       L.svf_simulate(C.byref(tr), 0, 1000, C.byref(res), WS, BIG, None),
+       L.svf_simulate(C.byref(tr), 0, 1 << 31, C.byref(res), WS, BIG, None),
+       L.svf_simulate_policies(C.byref(tr), 2, pol, 1000, outs, WS, BIG, None),
+       L.svf_volume_lower_bound(C.byref(tr), P1, None, WS, BIG, None),
+       L.svf_admit(0, 1000, 0, 500, P0, P0, P0, None, 1, 1, 40, P0, P0, P1, None, None, None, WS, BIG, None),
+       L.svf_sort_words(5000, P0, P1, 0, 64, WS, BIG, None)]
+print(",".join(str(r) for r in rcs))
+"""
+
+
+def test_compute_calls_return_ecuda_without_a_device(svf_lib):
+    """No CPU fallback: with no CUDA device visible every compute entry point returns SVF_ECUDA (3)
+    and touches none of its buffers.  Run in a child process with CUDA_VISIBLE_DEVICES empty, so the
+    test says the same on the GPU box."""
+    import subprocess
+    import sys
+    from paper_2606_22327_b200 import build
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="")
+    out = subprocess.run([sys.executable, "-c", _NO_DEVICE_SCRIPT.format(root=ROOT, lib=build.LIB)], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr
+    assert out.stdout.strip() == ",".join(["3"] * 7), out.stdout

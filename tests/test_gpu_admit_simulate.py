@@ -370,6 +370,29 @@ def test_admit_wide_budget_takes_the_sorted_array_kernel(B, oracle):
         assert k == 4000                                  # everything fits
 
 
+def test_admit_prefix_bisection_and_its_handover(B, oracle):
+    """The bisection kernel holds running + the first (8192 - n_run) candidates.  Cases: the answer
+    inside that window (tight budgets, every policy); the window exhausted with more waiting ->
+    the serial kernels take over from the running order it wrote (32-bit slots and 64-bit path);
+    n_run above 4096 -> the device-wide sort of the running set + the serial kernels; a running
+    set that is infeasible on its own admits nobody."""
+    for n_wait, n_run, M in ((9000, 0, 150_000), (9000, 700, 1_500_000), (30_000, 4096, 8_000_000),
+                             (8192, 0, 60_000), (8193, 0, 10 ** 7), (5000, 3192, 6_000_000)):
+        st = _admit_state(n_wait * 7 + n_run, n_wait, n_run, M)
+        ks = [_admit_both(B, oracle, policy, M, st) for policy in range(4)]
+        assert max(ks) > 0
+    st = _admit_state(5, 20_000, 100, 1_000_000)
+    assert _admit_both(B, oracle, 0, (1 << 30) - 1, st) == 20_000      # window exhausted: slot kernels finish
+    assert _admit_both(B, oracle, 3, 1 << 40, st) == 20_000            # ... and the 64-bit kernel
+    k = _admit_both(B, oracle, 0, 10_000_000, st)                      # handed over AND then blocked
+    assert 8092 < k < 20_000
+    st = _admit_state(6, 3000, 4097, 8_000_000)
+    assert _admit_both(B, oracle, 0, 8_000_000, st) > 0                # n_run > 4096: serial path
+    w_s, w_o, w_a, w_bit, r_kv, r_rem = _admit_state(7, 500, 50, 1_000_000)
+    r_kv = r_kv.copy(); r_kv[0] = 999_990                              # running set alone already over M at its first completion
+    assert _admit_both(B, oracle, 0, 1_000_000, (w_s, w_o, w_a, w_bit, r_kv, r_rem)) == 0
+
+
 def test_admit_everything_fits_and_nothing_fits(B, oracle):
     st = _admit_state(1, 300, 40, 10 ** 6)
     assert _admit_both(B, oracle, 0, 10 ** 12, st) == 300           # whole queue admitted
