@@ -350,6 +350,8 @@ __global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wa
     if (*handoff == 0) return;               // data error or infeasible running set: k_admit has answered
     const int tid = threadIdx.x;
     const int Mi = (int)M;
+    const uint32_t one = n_run >= 0 ? 1u : 0u;           // 1, but not to the compiler (SVF_ACC_GE)
+    (void)one;
     const uint64_t* __restrict__ rsorted = rsorted_direct ? rsorted_direct : rplan->result;
     const uint64_t* __restrict__ wsorted = wplan->result;
     const int R = (int)n_run;
@@ -377,14 +379,14 @@ __global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wa
         const int fh = ohi;
         const uint32_t oh = (uint32_t)ohi, fhu = (uint32_t)fh;
         const uint32_t Kc = (uint32_t)sh - (uint32_t)Mi, add = (uint32_t)sh;
-        uint32_t acc = 0, dm = 0;
+        uint32_t acc = 0, acc1 = 0, dm = 0;
         int viol = INT_MIN;
         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;
         const int g4 = (kmax + 3) >> 2;
         const bool use_ext = hw > REGCAP;
         SVF_SLOT_GROUPS(g4, SVF_EVAL)
-        const uint32_t low = dm ? (dm & (0u - dm)) : (1u << (4 * g4));
-        int fkey = low < (1u << K) ? (int)((low << TSHIFT) | (uint32_t)tid) : INT_MAX;
+        const uint32_t dmx = dm | (1u << (4 * g4));          // sentinel: the first slot past the groups in use (16 = none)
+        int fkey = (int)(((dmx & (0u - dmx)) << TSHIFT) | (uint32_t)tid);
         int eidx = INT_MAX;
         if (use_ext) {
             for (int q = REGCAP + tid; q < hw; q += THREADS) {
@@ -396,12 +398,13 @@ __global__ void __launch_bounds__(THREADS) k_admit_slots(int64_t M, int64_t n_wa
                 if (x >> 31) eidx = eidx < q ? eidx : q;
             }
         }
+        acc += acc1;
         reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
         const int Ah = sh + ohi + (int)acc;
         if (viol > 0 || Ah > Mi) break;                      // blocked head: nobody may bypass it
         const uint32_t Bh = (uint32_t)Ah + fhu;
         int idx;
-        if (fkey != INT_MAX) {
+        if (fkey < (1 << (K + TSHIFT))) {
             const int ik = 31 - __clz(fkey >> TSHIFT);
             const bool mine = (fkey & (THREADS - 1)) == tid;
             idx = (ik << TSHIFT) + (fkey & (THREADS - 1));

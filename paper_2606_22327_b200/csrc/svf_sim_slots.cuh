@@ -157,7 +157,7 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
 // QREG: shared memory holds the (s, o) records by rank and the bitmap mirror; the ext slots
 // (touched only when more than 32*K requests run at once) live in a global slot per CTA
 constexpr int QREG_RANKS = 1024;
-constexpr size_t QREG_SMEM_BYTES = (size_t)QREG_RANKS * 8 + 32 * 4;
+constexpr size_t QREG_SMEM_BYTES = (size_t)QREG_RANKS * 8 + 32 * 4 + 32 * 8;   // (s, o) by rank, bitmap mirror, output buffer
 __host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
 
 // one reduction round over the group: a summed (mod 2^32), b maxed, c minned; uniform afterwards
@@ -253,9 +253,25 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 // kernel (k_sim_slots here, k_admit_slots in svf_admit.cu): slots f[], B[], c[]; the head's t1 =
 // t + 1, oh = o_h, fh / fhu = f_h, Kc = s_h - t - M, add = s_h - t; accumulators acc, viol, dm
 // (evaluation) and wmax, minge (blocked head); cntE / cntU under COUNT.
+#ifndef SVF_EVAL_FMA
+#define SVF_EVAL_FMA 1
+#endif
+#if SVF_EVAL_FMA
+// condition (1) on the FMA pipe: the alu pipe is the busy one (ISETP, VIADDMNMX, SHF, IADD3 take one
+// warp instruction per two cycles per scheduler, and so does the fma pipe, which is nearly idle
+// here), so the predicated accumulate is an IMAD by a register that holds 1 (`one`: a run-time
+// value, or ptxas would turn it back into SEL + IADD3 on the alu pipe); two accumulators
+#define SVF_ACC_GE(k) {                                                                        \
+    const uint32_t tmp_ = c[k] + fhu;                                  \
+    if ((k) & 1) asm("{\n\t.reg .pred p;\n\tsetp.ge.s32 p, %1, %2;\n\t@p mad.lo.u32 %0, %3, %4, %0;\n\t}" : "+r"(acc1) : "r"(f[k]), "r"(fh), "r"(tmp_), "r"(one)); \
+    else         asm("{\n\t.reg .pred p;\n\tsetp.ge.s32 p, %1, %2;\n\t@p mad.lo.u32 %0, %3, %4, %0;\n\t}" : "+r"(acc) : "r"(f[k]), "r"(fh), "r"(tmp_), "r"(one)); \
+}
+#else
+#define SVF_ACC_GE(k) { if (f[k] >= fh) acc += c[k] + fhu; }
+#endif
 #define SVF_EVAL(k) {                                                                          \
     const uint32_t x = (uint32_t)f[k] - t1;                            \
-    if (f[k] >= fh) acc += c[k] + fhu;                                 \
+    SVF_ACC_GE(k)                                                      \
     if (x < oh) {                                                      \
         viol = __viaddmax_s32((int)B[k], (int)Kc, viol);               \
         B[k] += add + (uint32_t)f[k];                                  \
@@ -274,6 +290,17 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
             if (COUNT) cntU -= 1;                                      \
         }                                                              \
         if (f[k] >= fh) minge = f[k] < minge ? f[k] : minge;           \
+    }
+// the same when only condition (2) failed: the end of a violated (1) (minge) is not needed
+#define SVF_BLOCK2(k) {                                                                        \
+        const uint32_t x = (uint32_t)f[k] - t1;                        \
+        if (x < oh) {                                                  \
+            B[k] -= add + (uint32_t)f[k];                              \
+            const int v = (int)(B[k] + Kc), d = (int)x + 1;            \
+            const int w = v < d ? v : d;                               \
+            wmax = w > wmax ? w : wmax;                                \
+            if (COUNT) cntU -= 1;                                      \
+        }                                                              \
     }
 #define SVF_PUT(k) if (mine) { f[k] = fh; B[k] = Bh; c[k] = add; }
 
@@ -312,8 +339,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
     uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QREG_RANKS * 8);  // QREG only
+    int2* obuf = reinterpret_cast<int2*>(dyn_smem + (size_t)QREG_RANKS * 8 + 32 * 4);  // QREG only: (rank, start) of the last <= 32 admissions
     const int Mi = (int)g.M;
     const int64_t n_items = g.I * g.n_policies;
+    const uint32_t one = g.n_policies > 0 ? 1u : 0u;      // 1, but not to the compiler (SVF_ACC_GE)
+    (void)one;
 
     while (true) {
         if (tid == 0) inst_s = (long long)atomicAdd(g.work_ctr, 1ull);
@@ -351,6 +381,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
             max_a = ai > max_a ? ai : max_a;
+            // QREG: the (s, o) of every request by RANK in shared memory, once per instance (the presort
+            // wrote a permutation of [0, n) whatever the data was), so that picking a head never waits
+            // for global memory
+            if (QREG) qrec[io.rank[base + i] & (QREG_RANKS - 1)] = make_int2(si, oi);
         }
         flags = G::or_u32(flags, scratch, parity);
         sum_o = G::sum_i64(sum_o, scratch, parity);
@@ -378,10 +412,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             int32_t* __restrict__ out_finish = io.finish + base;
             uint32_t* out_lat = io.lat + base;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
-            uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32)
-            if (QREG) {
-                qbits[lane] = 0;
-            } else {
+            uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32); the register is the truth
+            if (!QREG) {
                 for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
                 for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
             }
@@ -391,11 +423,12 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             for (int k = 0; k < K; ++k) { f[k] = 0; B[k] = 0; c[k] = 0; }
 
             // arrival window: lane l holds request wb + l
-            int wb = 0, aw, sw, ow, rw;
+            int wb = 0, aw, sw = 0, ow = 0, rw;
             auto load_window = [&]() {
                 const int idx = wb + lane;
                 const bool in = idx < n;
-                aw = in ? a[idx] : INT_MAX; sw = in ? s[idx] : 0; ow = in ? o[idx] : 0;
+                aw = in ? a[idx] : INT_MAX;
+                if (!QREG) { sw = in ? s[idx] : 0; ow = in ? o[idx] : 0; }
                 rw = in ? (int)rnk[idx] : INT_MAX;
             };
             load_window();
@@ -405,17 +438,24 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             };
             // output buffer: admission number m sits in lane m % 32 of warp 0 until 32 are there
             // (QREG: b_id holds the RANK; id and arrival are looked up when the buffer is written)
+            // (QREG: (rank, start) go to a 32-entry buffer in shared memory; id, arrival and o are looked
+            // up when the buffer is written)
             int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
             auto flush = [&](int count) {
+                if (QREG) __syncwarp();
                 if (wrp == 0 && lane < count) {
                     int id = b_id, lat = b_lat;
-                    if (QREG) { id = (int)ord[b_id]; lat = b_f - a[id]; }
+                    if (QREG) {
+                        const int2 e = obuf[lane];
+                        id = (int)ord[e.x]; b_t = e.y; b_f = e.y + qrec[e.x].y; lat = b_f - a[id];
+                    }
                     if (want_start) out_start[id] = b_t;
                     if (want_finish) out_finish[id] = b_f;
                     if (want_p99) out_lat[id] = (uint32_t)lat;
                     tel += lat;
                     mk = b_f > mk ? b_f : mk;
                 }
+                if (QREG) __syncwarp();
             };
             G::sync();
 
@@ -423,6 +463,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             head.r = INT_MAX; head.s = head.o = head.id = head.a = 0;
             second = head;
             int next = 0, started = 0, hw = 0;
+            uint32_t hrest = 0; int hbase = 0;    // QREG: the head's bitmap word above the head, and its first rank
             int32_t t = a[0];
             int32_t t_lb = t;                     // first step at which the head must be (re)evaluated
 
@@ -436,9 +477,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                     const uint32_t m = __ballot_sync(FULL, v);
                     if (!m) break;
                     if (QREG) {
-                        // the owner's plain store of a cleared word comes before these atomics
-                        if (!arrived) __syncwarp();
-                        if (v) { qrec[rw] = make_int2(sw, ow); atomicOr(&qbits[rw >> 5], 1u << (rw & 31)); }
+                        // the arrivals of a step set their bits in a shared-memory copy of the bitmap
+                        if (!arrived) { qbits[lane] = qword; __syncwarp(); }
+                        if (v) atomicOr(&qbits[rw >> 5], 1u << (rw & 31));
                     } else {
                         // nobody may still be reading the bitmap for the previous step
                         if (!arrived) G::sync();
@@ -473,7 +514,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                         qword = qbits[lane];
                         const uint32_t nz = __ballot_sync(FULL, qword != 0u);
                         const int l0 = __ffs(nz) - 1;
-                        const int r0 = l0 * 32 + (__ffs(__shfl_sync(FULL, qword, l0)) - 1);
+                        const uint32_t w0 = __shfl_sync(FULL, qword, l0);
+                        const int r0 = l0 * 32 + (__ffs(w0) - 1);
+                        hbase = l0 * 32; hrest = w0 & (w0 - 1u);
                         if (r0 != head.r) {
                             const int2 v = qrec[r0];
                             head.r = r0; head.s = v.x; head.o = v.y;
@@ -493,7 +536,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                         const uint32_t t1 = (uint32_t)t + 1u, oh = (uint32_t)head.o, fhu = (uint32_t)fh;
                         const uint32_t Kc = (uint32_t)head.s - (uint32_t)t - (uint32_t)Mi;   // s_h - t - M (mod 2^32)
                         const uint32_t add = (uint32_t)head.s - (uint32_t)t;                  // A_j += s_h - t + f_j
-                        uint32_t acc = 0, dm = 0;
+                        uint32_t acc = 0, acc1 = 0, dm = 0;
                         int viol = INT_MIN;
                         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
                         const int g4 = (kmax + 3) >> 2;
@@ -501,8 +544,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                         SVF_SLOT_GROUPS(g4, SVF_EVAL)
                         // lowest free register slot of this thread as a one-hot bit (bit k of dm =
                         // slot k is dead); the group takes the lowest (slot, thread) pair
-                        const uint32_t low = dm ? (dm & (0u - dm)) : (1u << (4 * g4));
-                        int fkey = low < (1u << K) ? (int)((low << TSHIFT) | (uint32_t)tid) : INT_MAX;
+                        // (a sentinel bit marks the first slot past the groups in use; slot 16 = none)
+                        const uint32_t dmx = dm | (1u << (4 * g4));
+                        int fkey = (int)(((dmx & (0u - dmx)) << TSHIFT) | (uint32_t)tid);
                         int eidx = INT_MAX;
                         if (use_ext) {
                             for (int q = REGCAP + tid; q < hw; q += THREADS) {
@@ -519,6 +563,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                                 if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
                             }
                         }
+                        acc += acc1;
                         reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
                         if (COUNT) ++cntV;
                         const int Ah = head.s + head.o + (int)acc;        // exact: 0 <= A_h <= 2M < 2^31
@@ -527,7 +572,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                             // long the head stays blocked at least --------------------------------
                             int wmax = 0, minge = INT_MAX;
                             if (COUNT) ++cntBk;
-                            SVF_SLOT_GROUPS(g4, SVF_BLOCK)
+                            if (Ah > Mi) { SVF_SLOT_GROUPS(g4, SVF_BLOCK) } else { SVF_SLOT_GROUPS(g4, SVF_BLOCK2) }
                             if (use_ext) {
                                 for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                     const int e = q - REGCAP;
@@ -554,7 +599,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                         // ---- admitted: the update is already in place; write the head into a slot --
                         const uint32_t Bh = (uint32_t)Ah + fhu;
                         int idx;
-                        if (fkey != INT_MAX) {
+                        if (fkey < (1 << (K + TSHIFT))) {
                             const int ik = 31 - __clz(fkey >> TSHIFT);           // uniform
                             const bool mine = (fkey & (THREADS - 1)) == tid;
                             idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
@@ -578,20 +623,31 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                             peak = p2 > peak ? p2 : peak;
                         }
                         if (QREG) {
-                            if (lane == (head.r >> 5)) { qword &= ~(1u << (head.r & 31)); qbits[lane] = qword; }
-                            if (lane == (started & 31)) { b_id = head.r; b_t = t; b_f = fh; }
+                            const uint32_t hb = (uint32_t)head.r - (uint32_t)(lane << 5);
+                            if (hb < 32u) qword &= ~(1u << hb);
+                            obuf[started & 31] = make_int2(head.r, t);     // every lane, same value: one broadcast store
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
                             if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
                         }
-                        ++started; ++decisions;
+                        ++started;                                     // (decisions: the admissions are added at the end)
                         if ((started & 31) == 0) flush(32);
                         if (QREG) {
-                            // next head: the lowest set bit; its (s, o) come from shared memory
-                            const uint32_t nz = __ballot_sync(FULL, qword != 0u);
-                            if (!nz) { head.r = INT_MAX; break; }
-                            const int l0 = __ffs(nz) - 1;
-                            const int r = l0 * 32 + (__ffs(__shfl_sync(FULL, qword, l0)) - 1);
+                            // next head: the next set bit of the word the head came from (a uniform copy
+                            // of it, `hrest`), else the lowest set bit of the later words; its (s, o) come
+                            // from shared memory
+                            int r;
+                            if (hrest) {
+                                r = hbase + (__ffs(hrest) - 1);
+                                hrest &= hrest - 1u;
+                            } else {
+                                const uint32_t nz = __ballot_sync(FULL, qword != 0u);
+                                if (!nz) { head.r = INT_MAX; break; }
+                                const int l0 = __ffs(nz) - 1;
+                                const uint32_t w0 = __shfl_sync(FULL, qword, l0);
+                                hbase = l0 * 32; hrest = w0 & (w0 - 1u);
+                                r = hbase + (__ffs(w0) - 1);
+                            }
                             const int2 v = qrec[r];
                             head.r = r; head.s = v.x; head.o = v.y;
                         } else {
@@ -624,6 +680,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
                 t = tn;
             }
             flush(started & 31);
+            decisions += (uint32_t)started;
             if (want_p99) {                       // nearest rank ceil(0.99 n), 1-based (R13)
                 G::sync();
                 p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity);
