@@ -247,7 +247,16 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
 #define SVF_PUT4(ik, OP, k0)  if ((ik) & 2) { SVF_PUT2(ik, OP, k0 + 2) } else { SVF_PUT2(ik, OP, k0) }
 #define SVF_PUT8(ik, OP, k0)  if ((ik) & 4) { SVF_PUT4(ik, OP, k0 + 4) } else { SVF_PUT4(ik, OP, k0) }
+#ifndef SVF_PUT_SWITCH
+#define SVF_PUT_SWITCH 0
+#endif
+#if SVF_PUT_SWITCH
+#define SVF_PUT16(ik, OP)     switch (ik) { case 0: OP(0) break; case 1: OP(1) break; case 2: OP(2) break; case 3: OP(3) break; \
+    case 4: OP(4) break; case 5: OP(5) break; case 6: OP(6) break; case 7: OP(7) break; case 8: OP(8) break; case 9: OP(9) break; \
+    case 10: OP(10) break; case 11: OP(11) break; case 12: OP(12) break; case 13: OP(13) break; case 14: OP(14) break; default: OP(15) break; }
+#else
 #define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
+#endif
 
 // The per-slot operations of the passes.  They are macros over the LOCAL names of the calling
 // kernel (k_sim_slots here, k_admit_slots in svf_admit.cu): slots f[], B[], c[]; the head's t1 =
@@ -255,6 +264,9 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 // (evaluation) and wmax, minge (blocked head); cntE / cntU under COUNT.
 #ifndef SVF_EVAL_FMA
 #define SVF_EVAL_FMA 1
+#endif
+#ifndef SVF_EVAL_FMA_B
+#define SVF_EVAL_FMA_B 1
 #endif
 #if SVF_EVAL_FMA
 // condition (1) on the FMA pipe: the alu pipe is the busy one (ISETP, VIADDMNMX, SHF, IADD3 take one
@@ -274,7 +286,10 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     SVF_ACC_GE(k)                                                      \
     if (x < oh) {                                                      \
         viol = __viaddmax_s32((int)B[k], (int)Kc, viol);               \
-        B[k] += add + (uint32_t)f[k];                                  \
+        if (SVF_EVAL_FMA_B && ((k) & 3) == 1) {                        \
+            asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(B[k]) : "r"(f[k]), "r"(one));       \
+            asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(B[k]) : "r"(add), "r"(one));        \
+        } else B[k] += add + (uint32_t)f[k];                           \
         if (COUNT) cntU += 1;                                          \
     }                                                                  \
     dm = __funnelshift_l(x, dm, 1);                                    \
@@ -308,8 +323,11 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 // asked for 19 CTAs per SM it fits the kernel into 96 registers WITHOUT spills (21 warps per SM
 // resident) and the launch is 5 % faster; 20 also gives 96 registers but a slower schedule, 17-18
 // and 21 spill (all measured on configs[2], profiles/r01_kslots_full.md).
+#ifndef SVF_WARP_MIN_CTAS
+#define SVF_WARP_MIN_CTAS 19
+#endif
 template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
-__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_sim_slots(SlotArgs g)
+__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MIN_CTAS : 1) k_sim_slots(SlotArgs g)
 {
     static_assert(K == 16, "SVF_SLOT_GROUPS / SVF_PUT16 are written out for 16 register slots per thread");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
@@ -322,7 +340,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
     __shared__ int scratch[2][64];
     __shared__ int red[2][WARPS][3];
     __shared__ long long inst_s;
-    __shared__ uint32_t hist[256];
+    // the p99 selection's histogram: its own kilobyte, except under QREG where it reuses the (s, o)
+    // records (dead once the instance is simulated; one kilobyte less per CTA = one more CTA per SM)
+    __shared__ uint32_t hist_s[QREG ? 1 : 256];
+    uint32_t* hist = QREG ? reinterpret_cast<uint32_t*>(dyn_smem) : hist_s;
     int parity = 0, rparity = 0;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
 
@@ -424,12 +445,22 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
 
             // arrival window: lane l holds request wb + l
             int wb = 0, aw, sw = 0, ow = 0, rw;
+            // QREG (96 registers, none to spare): the rarely taken paths (window refill every 32 arrivals,
+            // output flush every 32 admissions) re-derive their pointers from (policy index, base)
+            // behind an opaque copy, so that no 64-bit pointer stays live across the hot loop
             auto load_window = [&]() {
                 const int idx = wb + lane;
                 const bool in = idx < n;
-                aw = in ? a[idx] : INT_MAX;
-                if (!QREG) { sw = in ? s[idx] : 0; ow = in ? o[idx] : 0; }
-                rw = in ? (int)rnk[idx] : INT_MAX;
+                if (QREG) {
+                    int pi_ = pi; long long b_ = base;
+                    asm volatile("" : "+r"(pi_), "+l"(b_));
+                    aw = in ? g.a[b_ + idx] : INT_MAX;
+                    rw = in ? (int)g.io[pi_].rank[b_ + idx] : INT_MAX;
+                } else {
+                    aw = in ? a[idx] : INT_MAX;
+                    sw = in ? s[idx] : 0; ow = in ? o[idx] : 0;
+                    rw = in ? (int)rnk[idx] : INT_MAX;
+                }
             };
             load_window();
             auto win_rec = [&](int l, int r) {
@@ -443,12 +474,22 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? 19 : 1) k_s
             int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
             auto flush = [&](int count) {
                 if (QREG) __syncwarp();
-                if (wrp == 0 && lane < count) {
-                    int id = b_id, lat = b_lat;
-                    if (QREG) {
+                if (QREG) {
+                    if (lane < count) {
+                        int pi_ = pi; long long b_ = base;
+                        asm volatile("" : "+r"(pi_), "+l"(b_));
+                        const PolicyIO& io_ = g.io[pi_];
                         const int2 e = obuf[lane];
-                        id = (int)ord[e.x]; b_t = e.y; b_f = e.y + qrec[e.x].y; lat = b_f - a[id];
+                        const int id = (int)io_.order[b_ + e.x];
+                        const int fin = e.y + qrec[e.x].y, lat = fin - g.a[b_ + id];
+                        if (io_.start) io_.start[b_ + id] = e.y;
+                        if (io_.finish) io_.finish[b_ + id] = fin;
+                        if (io_.p99) io_.lat[b_ + id] = (uint32_t)lat;
+                        tel += lat;
+                        mk = fin > mk ? fin : mk;
                     }
+                } else if (wrp == 0 && lane < count) {
+                    const int id = b_id, lat = b_lat;
                     if (want_start) out_start[id] = b_t;
                     if (want_finish) out_finish[id] = b_f;
                     if (want_p99) out_lat[id] = (uint32_t)lat;
