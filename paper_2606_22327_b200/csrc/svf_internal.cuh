@@ -87,14 +87,25 @@ void   sort_ws_carve(SortWs* w, void* base, int64_t n, int bit_lo, int bit_hi);
 int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int64_t n, int bit_lo,
              int bit_hi, cudaStream_t st, int64_t* launches);
 // Segmented sort of small segments in shared memory (one CTA per instance, max_instance <=
-// SEG_SORT_MAX): computes the priority keys from the trace and writes order[] (local id at
-// instance offset + rank), rank[] (rank of instance offset + local id) and, if req != nullptr,
-// the (s, o, id, a) records in priority order.  One launch.
+// SEG_SORT_MAX): for every policy of the call it computes the priority keys from the trace and writes
+// order[] (local id at instance offset + rank), rank[] (rank of instance offset + local id) and, if
+// req != nullptr, the (s, o, id, a) records in priority order.  ONE launch for all policies.
 constexpr int SEG_SORT_MAX = 4096;
-int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
-                  const int32_t* s, const int32_t* o, const int32_t* okey /* key lengths or NULL */,
-                  const int32_t* a, const uint8_t* bit, int32_t O0, int32_t O1, uint32_t* order, uint32_t* rank,
-                  int4* req, cudaStream_t st, int64_t* launches);
+constexpr int SEG_SORT_MAX_POLICIES = 8;
+struct SegSortArgs {
+    int64_t I, N;
+    int cap;                         // filled in by seg_sort_keys
+    const int64_t* off;
+    const int32_t *s, *o, *okey /* key lengths or NULL */, *a;
+    const uint8_t* bit;
+    int32_t O0, O1;
+    int n_policies;
+    int policy[SEG_SORT_MAX_POLICIES];
+    uint32_t* order[SEG_SORT_MAX_POLICIES];
+    uint32_t* rank[SEG_SORT_MAX_POLICIES];
+    int4* req[SEG_SORT_MAX_POLICIES];
+};
+int seg_sort_keys(const SegSortArgs& A, int64_t max_instance, cudaStream_t st, int64_t* launches);
 // copy plan->result to out unless it already is out
 int sort_result_to(const SortWs& w, uint64_t* out, int64_t n, cudaStream_t st, int64_t* launches);
 

@@ -686,6 +686,10 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     q.O0 = tr->O0; q.O1 = tr->O1;
     q.off = tr->offsets; q.a = tr->arrival; q.s = tr->prompt; q.o = tr->output; q.okey = tr->output_key; q.bit = tr->bit;
     q.n_policies = P;
+    const bool seg = N > 0 && tr->max_instance <= SEG_SORT_MAX;
+    SegSortArgs sa;
+    sa.I = I; sa.N = N; sa.cap = 0; sa.off = tr->offsets; sa.s = tr->prompt; sa.o = tr->output; sa.okey = tr->output_key;
+    sa.a = tr->arrival; sa.bit = tr->bit; sa.O0 = tr->O0; sa.O1 = tr->O1; sa.n_policies = P;
     for (int k = 0; k < P; ++k) {
         const svf_result_t* out = &outs[k];
         PolicyIO& io = q.io[k];
@@ -696,13 +700,8 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
         io.rounds = out->rounds; io.decisions = out->decisions; io.p99 = out->p99_latency;
         io.makespan = out->makespan; io.status = out->status;
         io.lat = w.lat[k];
-        if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
-            // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance
-            if (seg_sort_keys(policies[k], I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, tr->output_key, tr->arrival,
-                              tr->bit, tr->O0, tr->O1, w.order[k], w.rank[k], c.qreg ? nullptr : w.req[k], st,
-                              &g_launches_sim))
-                return SVF_ECUDA;
-        } else if (N > 0) {
+        sa.policy[k] = policies[k]; sa.order[k] = w.order[k]; sa.rank[k] = w.rank[k]; sa.req[k] = c.qreg ? nullptr : w.req[k];
+        if (!seg && N > 0) {
             SimArgs g;
             g.I = I; g.N = N; g.M = M; g.max_instance = tr->max_instance;
             g.policy = policies[k]; g.O0 = tr->O0; g.O1 = tr->O1; g.sb = c.sb;
@@ -718,6 +717,9 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
             ++g_launches_sim;
         }
     }
+    // small instances: keys + stable radix sort + rank in shared memory, one CTA per instance, every
+    // policy of the call in ONE launch
+    if (seg && seg_sort_keys(sa, tr->max_instance, st, &g_launches_sim)) return SVF_ECUDA;
     prof_mark(1, st);
 
     // ---- phase B: one persistent launch over P x I work items -------------------------------------
@@ -811,10 +813,11 @@ extern "C" int svf_volume_lower_bound(const svf_trace_t* tr, int64_t* lb_out, in
     }
     // volumes ascending = the SVF order under the TRUE lengths (no predicted keys here)
     if (N > 0 && tr->max_instance <= SEG_SORT_MAX) {
-        if (seg_sort_keys(SVF_SVF, I, N, tr->max_instance, tr->offsets, tr->prompt, tr->output, nullptr,
-                          tr->prompt /* a is not read by the SVF key */, nullptr, 0, 0, w.order[0], w.rank[0], nullptr, st,
-                          &g_launches_sim))
-            return SVF_ECUDA;
+        SegSortArgs sa;
+        sa.I = I; sa.N = N; sa.cap = 0; sa.off = tr->offsets; sa.s = tr->prompt; sa.o = tr->output; sa.okey = nullptr;
+        sa.a = tr->prompt /* not read: no records are written */; sa.bit = nullptr; sa.O0 = 0; sa.O1 = 0; sa.n_policies = 1;
+        sa.policy[0] = SVF_SVF; sa.order[0] = w.order[0]; sa.rank[0] = w.rank[0]; sa.req[0] = nullptr;
+        if (seg_sort_keys(sa, tr->max_instance, st, &g_launches_sim)) return SVF_ECUDA;
     } else if (N > 0) {
         SimArgs g;
         g.I = I; g.N = N; g.M = 0; g.max_instance = tr->max_instance;

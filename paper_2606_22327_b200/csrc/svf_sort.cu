@@ -340,13 +340,7 @@ __global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan-
 // 12-13 B read + 8 B (24 B with records) written per request, against 8 + 16 B per executed pass
 // of the device-wide sort.
 template <int IPT>
-__global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I, int64_t N, int cap,
-                                                           const int64_t* __restrict__ off,
-                                                           const int32_t* __restrict__ s, const int32_t* __restrict__ o,
-                                                           const int32_t* __restrict__ okey,
-                                                           const int32_t* __restrict__ a, const uint8_t* __restrict__ bit,
-                                                           int32_t O0, int32_t O1, uint32_t* __restrict__ order,
-                                                           uint32_t* __restrict__ rank, int4* __restrict__ req)
+__global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(SegSortArgs A)
 {
     static_assert(SORT_THREADS == SORT_RADIX, "one thread per digit in the scans");
     constexpr int WARPS = SORT_THREADS / 32;
@@ -356,39 +350,62 @@ __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(int policy, int64_t I
     __shared__ uint32_t warp_tot[WARPS];
     __shared__ uint32_t kor_s;
     const int tid = threadIdx.x;
-    for (int64_t j = blockIdx.x; j < I; j += gridDim.x) {
-        const int64_t base = off[j], n64 = off[j + 1] - base;
-        if (n64 <= 0 || n64 > cap || base < 0 || base + n64 > N) continue;   // the simulator reports the layout error
+    const int cap = A.cap;
+    const int32_t* __restrict__ s = A.s;
+    const int32_t* __restrict__ o = A.o;
+    const int32_t* __restrict__ a = A.a;
+    const int32_t* __restrict__ klen = A.okey ? A.okey : A.o;     // the length the SVF / SJF key sees
+    for (int64_t j = blockIdx.x; j < A.I; j += gridDim.x) {
+        const int64_t base = A.off[j], n64 = A.off[j + 1] - base;
+        if (n64 <= 0 || n64 > cap || base < 0 || base + n64 > A.N) continue;   // the simulator reports the layout error
         const int n = (int)n64;
-        if (tid == 0) kor_s = 0;
-        __syncthreads();
-        uint64_t* buf0 = seg_buf;
-        uint64_t* buf1 = seg_buf + cap;
-        uint32_t kor = 0;
-        for (int i = tid; i < n; i += SORT_THREADS) {
-            const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)bit[base + i] : 0u;
-            const uint32_t key = (uint32_t)priority_key(policy, s[base + i], (okey ? okey : o)[base + i], a[base + i], b, O0, O1);
-            buf0[i] = ((uint64_t)key << 32) | (uint32_t)i;
-            kor |= key;
+        // every policy of the call on this instance: the trace is read from HBM once (the later
+        // policies hit L1 / L2) and the call pays one launch tail instead of one per policy
+        for (int q = 0; q < A.n_policies; ++q) {
+            const int policy = A.policy[q];
+            uint32_t* __restrict__ order = A.order[q];
+            uint32_t* __restrict__ rank = A.rank[q];
+            int4* __restrict__ req = A.req[q];
+            if (policy == SVF_FCFS) {
+                // key = arrival and the input IS in (arrival, id) order (an instance whose arrivals
+                // decrease is rejected by the simulator): the priority order is the identity
+                for (int p = tid; p < n; p += SORT_THREADS) {
+                    order[base + p] = (uint32_t)p;
+                    rank[base + p] = (uint32_t)p;
+                    if (req) req[base + p] = make_int4(s[base + p], o[base + p], p, a[base + p]);
+                }
+                continue;
+            }
+            if (tid == 0) kor_s = 0;
+            __syncthreads();
+            uint64_t* buf0 = seg_buf;
+            uint64_t* buf1 = seg_buf + cap;
+            uint32_t kor = 0;
+            for (int i = tid; i < n; i += SORT_THREADS) {
+                const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)A.bit[base + i] : 0u;
+                const uint32_t key = (uint32_t)priority_key(policy, s[base + i], klen[base + i], 0, b, A.O0, A.O1);
+                buf0[i] = ((uint64_t)key << 32) | (uint32_t)i;
+                kor |= key;
+            }
+            kor = __reduce_or_sync(0xffffffffu, kor);
+            if ((tid & 31) == 0 && kor) atomicOr(&kor_s, kor);
+            __syncthreads();
+            const uint32_t kall = kor_s;
+            const int bits = kall ? 32 - __clz(kall) : 0;
+            const int npass = (bits + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
+            const int ipt = (n + SORT_THREADS - 1) / SORT_THREADS;
+            for (int p = 0; p < npass; ++p) {
+                seg_pass<SORT_THREADS, IPT>(buf0, buf1, n, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
+                uint64_t* t = buf0; buf0 = buf1; buf1 = t;
+            }
+            for (int p = tid; p < n; p += SORT_THREADS) {
+                const uint32_t id = (uint32_t)buf0[p];
+                order[base + p] = id;
+                rank[base + id] = (uint32_t)p;
+                if (req) req[base + p] = make_int4(s[base + id], o[base + id], (int)id, a[base + id]);
+            }
+            __syncthreads();
         }
-        kor = __reduce_or_sync(0xffffffffu, kor);
-        if ((tid & 31) == 0 && kor) atomicOr(&kor_s, kor);
-        __syncthreads();
-        const uint32_t kall = kor_s;
-        const int bits = kall ? 32 - __clz(kall) : 0;
-        const int npass = (bits + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
-        const int ipt = (n + SORT_THREADS - 1) / SORT_THREADS;
-        for (int p = 0; p < npass; ++p) {
-            seg_pass<SORT_THREADS, IPT>(buf0, buf1, n, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
-            uint64_t* t = buf0; buf0 = buf1; buf1 = t;
-        }
-        for (int p = tid; p < n; p += SORT_THREADS) {
-            const uint32_t id = (uint32_t)buf0[p];
-            order[base + p] = id;
-            rank[base + id] = (uint32_t)p;
-            if (req) req[base + p] = make_int4(s[base + id], o[base + id], (int)id, a[base + id]);
-        }
-        __syncthreads();
     }
 }
 
@@ -473,15 +490,13 @@ int sort_u64(const SortWs& w, const uint64_t* in, uint64_t* x, uint64_t* y, int6
     return (int)cudaGetLastError();
 }
 
-int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const int64_t* off,
-                  const int32_t* s, const int32_t* o, const int32_t* okey, const int32_t* a, const uint8_t* bit,
-                  int32_t O0, int32_t O1, uint32_t* order, uint32_t* rank, int4* req, cudaStream_t st,
-                  int64_t* launches)
+int seg_sort_keys(const SegSortArgs& A, int64_t max_instance, cudaStream_t st, int64_t* launches)
 {
-    if (I <= 0 || N <= 0) return 0;
-    if (max_instance > SEG_SORT_MAX) return (int)cudaErrorInvalidValue;
-    const int cap = (int)((max_instance > 0 ? max_instance : 1) + 1) / 2 * 2;
-    const size_t smem = (size_t)2 * cap * sizeof(uint64_t);
+    if (A.I <= 0 || A.N <= 0 || A.n_policies <= 0) return 0;
+    if (max_instance > SEG_SORT_MAX || A.n_policies > SEG_SORT_MAX_POLICIES) return (int)cudaErrorInvalidValue;
+    SegSortArgs B = A;
+    B.cap = (int)((max_instance > 0 ? max_instance : 1) + 1) / 2 * 2;
+    const size_t smem = (size_t)2 * B.cap * sizeof(uint64_t);
     // items per thread sized to the largest instance (registers: occupancy of small segments)
 #define SVF_SEG_LAUNCH(IPT)                                                                             \
     do {                                                                                                \
@@ -492,12 +507,11 @@ int seg_sort_keys(int policy, int64_t I, int64_t N, int64_t max_instance, const 
                 != cudaSuccess || per_sm < 1)                                                           \
             per_sm = 1;                                                                                 \
         int64_t grid = (int64_t)per_sm * sm_count();                                                    \
-        if (grid > I) grid = I;                                                                         \
-        k_seg_sort<IPT><<<(unsigned)grid, SORT_THREADS, smem, st>>>(policy, I, N, cap, off, s, o, okey, \
-                                                                    a, bit, O0, O1, order, rank, req);  \
+        if (grid > B.I) grid = B.I;                                                                     \
+        k_seg_sort<IPT><<<(unsigned)grid, SORT_THREADS, smem, st>>>(B);                                 \
     } while (0)
-    if (cap <= 4 * SORT_THREADS) SVF_SEG_LAUNCH(4);
-    else if (cap <= 8 * SORT_THREADS) SVF_SEG_LAUNCH(8);
+    if (B.cap <= 4 * SORT_THREADS) SVF_SEG_LAUNCH(4);
+    else if (B.cap <= 8 * SORT_THREADS) SVF_SEG_LAUNCH(8);
     else SVF_SEG_LAUNCH(16);
 #undef SVF_SEG_LAUNCH
     ++*launches;
