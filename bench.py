@@ -48,9 +48,27 @@ OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
 # HBM bytes per request and policy the same kernel must move: a, s, o (12) + rank (4) + order (4) +
 # start, finish (8) + latency for the p99 selection (4 written, 4 read back)
 SIM_BYTES_PER_REQUEST = 36
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/r01_kslots_full.md (one launch = four policies)
-SIM_DRAM_TRAFFIC_BYTES = 515.1e6
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload come from the
+# committed `ncu --set full` summary of the same command (never from a run under the profiler here)
+SIM_PROFILE = os.path.join("profiles", "r02_kslots_full.md")
+
+
+def profiled_dram_traffic():
+    """(bytes per k_sim_slots launch, source) read from the committed ncu summary, or (None, why)."""
+    path = os.path.join(ROOT, SIM_PROFILE)
+    try:
+        rd = wr = None
+        for line in open(path):
+            f = [x.strip() for x in line.split("|")]
+            if len(f) >= 4 and f[1] == "dram__bytes_read.sum":
+                rd = float(f[3]) * {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0}[f[2]]
+            if len(f) >= 4 and f[1] == "dram__bytes_write.sum":
+                wr = float(f[3]) * {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0}[f[2]]
+        if rd is not None and wr is not None:
+            return rd + wr, f"{SIM_PROFILE} (dram__bytes_read.sum + dram__bytes_write.sum of one launch)"
+    except OSError:
+        pass
+    return None, f"{SIM_PROFILE} not found"
 
 
 def parse_args():
@@ -65,6 +83,7 @@ def parse_args():
     ap.add_argument("--e2e-chunks", type=int, default=8, help="instance chunks (streams) of the end-to-end leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel and per-config extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-oracle-extras", action="store_true", help="extras without the oracle timed beside each config")
     return ap.parse_args()
 
 
@@ -168,7 +187,7 @@ def run_reference(args):
     from oracle import svf_ref
     svf_ref.build()
     threads = min(os.cpu_count() or 1, svf_ref.max_threads())
-    n_inst = min(args.instances, 1024)            # bounded sample of the same workload
+    n_inst = args.instances                        # the same batch as the repo arm's rank 0 (about 1.5 s per step on 16 cores)
     sample = T.config3(n_instances=n_inst, n=args.requests, lam=args.lam)
     rs = sample.request_steps * len(POLICIES)
     for _ in range(max(args.warmup, 0) and 1):
@@ -178,7 +197,8 @@ def run_reference(args):
         oracle_step(svf_ref, sample, threads)
     dt = time.perf_counter() - t0
     val = rs * args.steps / dt
-    desc = f"{n_inst} of {args.instances} instances x {args.requests} requests x 4 policies per step"
+    desc = (f"all {n_inst} instances x {args.requests} requests x 4 policies per step, instance-parallel over {threads} "
+            f"host threads (nproc {os.cpu_count()})")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
@@ -309,6 +329,14 @@ def run_ours(args):
         return int(host_out[0][0]["total_latency"][0])
 
     e2e_step()
+    # the chunked, eight-stream leg must give what the single call gave: every policy, every field
+    for i in range(len(POLICIES)):
+        for k in B.RESULT_FIELDS:
+            n_k = batch.n_requests if k in ("start", "finish") else batch.n_instances
+            whole = getattr(outs[i], k)[:n_k].cpu()
+            parts = torch.cat([host_out[c][i][k][: (subs[c].n_requests if k in ("start", "finish") else subs[c].n_instances)]
+                               for c in range(n_chunks)])
+            assert torch.equal(whole, parts), f"end-to-end leg differs from the single call: policy {POLICY_NAMES[i]}, field {k}"
     barrier()
     te0 = time.perf_counter()
     n_e2e = max(2, min(args.steps, 5))
@@ -340,6 +368,7 @@ def run_ours(args):
     peak_ops, peak_src = alu_peak(torch, dev)
     sim_bytes = SIM_BYTES_PER_REQUEST * batch.n_requests * len(POLICIES)
     achieved = ops_per_launch / (sim_ms * 1e-3)
+    traffic, traffic_src = profiled_dram_traffic()
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -354,8 +383,9 @@ def run_ours(args):
         "gpu_launches": launches_all,
         "roofline": {"kernel": "k_sim_slots (persistent simulator, phase B)", "bound": "alu",
                      "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "Tlane-op/s",
-                     "frac": achieved / peak_ops, "traffic": SIM_DRAM_TRAFFIC_BYTES,
+                     "frac": achieved / peak_ops, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": peak_src,
+                     "frac_of_integer_pipe_rate": achieved / (peak_ops / 2),   # the alu pipe alone issues every other cycle
                      "algorithmic_ops_per_launch": ops_per_launch,
                      "entries_examined_per_launch": E,
                      "entries_updated_per_launch": U,
@@ -368,9 +398,11 @@ def run_ours(args):
                              "sees the trace once (DESIGN.md 6); 'kernels' lists the HBM-bound pieces"},
     }
     peak = hbm_peak
+    line["fingerprint_fnv1a64"] = T.trace_fingerprint(batch)
     if not args.no_extras:
         line["kernels"] = kernel_extras(B, torch, dev, peak)
-        line["configs"] = config_extras(B, torch, dev)
+        line["admit_sweep"] = admit_sweep(B, torch, dev, peak)
+        line["configs"] = config_extras(B, torch, dev, args, with_oracle=not (args.no_oracle_extras or args.no_cpu_baseline))
         line["ratio_to_lower_bound"] = bound_extras(B, torch, dev, args)
         # the paper's own metrics on the bench batch, per policy, this rank
         from paper_2606_22327_b200 import report as RP
@@ -420,38 +452,162 @@ def kernel_extras(B, torch, dev, peak):
     out.append({"kernel": "svf_sort_words (n=2^26, key bits [32,64), 4 passes executed)", "ms": ms,
                 "achieved": bytes_sort / ms / 1e6, "unit": "GB/s", "frac": bytes_sort / ms / 1e6 / peak,
                 "algorithmic_bytes": bytes_sort, "words_per_sec": n / ms * 1e3})
-    del s, o, words, srt, wsb
-    # admission decisions at depth (BASELINE.json configs[3] laws): W waiting, R running
-    tr = T.config4(n=1 << 18)
-    w = [torch.from_numpy(x).to(dev) for x in (tr.prompt, tr.output, tr.arrival, tr.bit)]
-    r_rem = torch.arange(1, 1025, dtype=torch.int32, device=dev) * 2
-    r_kv = torch.full((1024,), 200, dtype=torch.int32, device=dev)
-    res = B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem)
-    wsa = torch.empty(B.svf_admit_workspace_bytes(1 << 18, 1024), dtype=torch.uint8, device=dev)
-    ms = _time_cuda(torch, lambda: B.svf_admit(B.SVF, tr.M, 0, *w, tr.O0, tr.O1, r_kv, r_rem, ws=wsa, out=res))
-    k = int(res.n_admitted.item())
-    out.append({"kernel": "svf_admit (W=2^18 waiting, R=1024 running, policy svf)", "ms": ms, "admitted": k,
-                "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": (1 << 18) / ms * 1e3})
     return out
 
 
-def config_extras(B, torch, dev):
-    """The other BASELINE.json configs, device-resident, SVF policy: context, not the headline."""
+def admit_sweep(B, torch, dev, peak):
+    """the stateless admission decision at depth.  W waiting requests (BASELINE.json
+    configs[3] laws) x R running requests (a loaded engine: the running set alone peaks at 0.8 M),
+    M = 1e6, policy SVF; the phase split comes from CUDA events the library records on the stream."""
     res = []
-    cases = [("configs[1] single online trace n=2000", T.config2(0)),
-             ("configs[3] single instance n=200000", T.config4()),
-             ("configs[4] 256x5000 M=200k p=0.05", T.config5(M=200_000, p_flip=0.05))]
-    for name, tr in cases:
-        d = B.DeviceTrace.from_host(tr, device=dev)
-        ws = torch.empty(B.svf_simulate_workspace_bytes(d), dtype=torch.uint8, device=dev)
-        for pol in (B.SVF, B.SVF_1BIT):
-            out = B.SimOut.alloc(d)
-            ms = _time_cuda(torch, lambda: B.svf_simulate(d, pol, out=out, ws=ws), reps=3)
-            res.append({"config": name, "policy": POLICY_NAMES[pol], "ms": ms,
-                        "request_steps_per_sec": tr.request_steps / ms * 1e3,
-                        "decisions_per_sec": int(out.decisions.sum().item()) / ms * 1e3,
-                        "total_latency": int(out.total_latency.sum().item())})
+    M = 1_000_000
+    for W in (1 << 10, 1 << 14, 1 << 18):
+        for R in (256, 1024, 4096):
+            w_s, w_o, w_a, w_bit, r_kv, r_rem = T.admit_state(W + R, W, R, M)
+            d = [torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in (w_s, w_o, w_a, w_bit, r_kv, r_rem)]
+            ws = torch.empty(B.svf_admit_workspace_bytes(W, R), dtype=torch.uint8, device=dev)
+            out = B.svf_admit(B.SVF, M, 0, d[0], d[1], d[2], d[3], 179, 887, d[4], d[5], ws=ws)
+            call = lambda: B.svf_admit(B.SVF, M, 0, d[0], d[1], d[2], d[3], 179, 887, d[4], d[5], ws=ws, out=out)
+            ms = _time_cuda(torch, call, reps=10)
+            B.set_profiling(True)
+            ph = []
+            for _ in range(5):
+                call()
+                ph.append(B.admit_phase_ms())
+            B.set_profiling(False)
+            ph = np.array(ph).mean(axis=0)
+            k = int(out.n_admitted.item())
+            # what the call must move: validation + keys read s, o, a (12 B) and write the packed word
+            # (8 B); the sort reads the words once for its histograms and reads + writes them once per
+            # executed pass (26-bit keys: four 8-bit passes over [32, 64)); the sorted words are copied
+            # out (16 B); the admission reads the running set and the first candidates (12 B each)
+            algo = W * (12 + 8 + 8 + 16 * 4 + 16) + (R + min(W, 8192 - R)) * 12
+            res.append({"W": W, "R": R, "ms": ms, "admitted": k, "launches": B.last_launch_count(1),
+                        "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": W / ms * 1e3,
+                        "phase_ms": {"keys_and_validation": float(ph[0]), "sorts": float(ph[1]), "admission": float(ph[2]),
+                                     "whole_call_under_events": float(ph[3])},
+                        "roofline": {"bound": "hbm", "achieved": algo / ms / 1e6, "peak": peak, "unit": "GB/s",
+                                     "frac": algo / ms / 1e6 / peak, "algorithmic_bytes": algo,
+                                     "note": "a chain of ~14 small launches: launch latency, not bandwidth, sets the time at these sizes"}})
     return res
+
+
+def _oracle_ms(svf_ref, tr, policy, threads):
+    t0 = time.perf_counter()
+    r = svf_ref.simulate(tr, policy, n_threads=threads)
+    return 1e3 * (time.perf_counter() - t0), r
+
+
+def config_extras(B, torch, dev, args, with_oracle=True):
+    """Every BASELINE.json config at its stated size, device resident, with the oracle timed beside it
+    on the host cores of the same box: one core for the single-instance configs, all
+    cores plus the one-core figure (on a sample) for the batched ones.  Context, not the headline."""
+    svf_ref, threads = None, 1
+    if with_oracle:
+        from oracle import svf_ref
+        svf_ref.build()
+        threads = min(os.cpu_count() or 1, svf_ref.max_threads())
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    info = {"nproc": os.cpu_count(), "oracle_threads_all_cores": threads, "entries": []}
+
+    def gpu_run(tr, pols):
+        d = B.DeviceTrace.from_host(tr, device=dev)
+        outs = [B.SimOut.alloc(d) for _ in pols]
+        ws = torch.empty(B.svf_simulate_policies_workspace_bytes(d, len(pols)), dtype=torch.uint8, device=dev)
+        ms = _time_cuda(torch, lambda: B.svf_simulate_policies(d, pols, outs=outs, ws=ws), reps=3, flush=flush)
+        return ms, outs
+
+    def entry(name, tr, pols, ms, outs, oracle=None):
+        e = {"config": name, "policies": [POLICY_NAMES[p] for p in pols], "gpu_ms": ms,
+             "instances": tr.n_instances, "requests": tr.n_requests, "M": tr.M, "fingerprint_fnv1a64": T.trace_fingerprint(tr),
+             "request_steps_per_sec": tr.request_steps * len(pols) / ms * 1e3,
+             "decisions_per_sec": sum(int(o.decisions.sum().item()) for o in outs) / ms * 1e3,
+             "total_latency": {POLICY_NAMES[p]: int(o.total_latency.sum().item()) for p, o in zip(pols, outs)}}
+        if oracle:
+            e["oracle"] = oracle
+        info["entries"].append(e)
+        return e
+
+    def check(name, pol, out, ref):
+        assert int(out.total_latency.sum().item()) == int(ref.total_latency.sum()), f"{name}: GPU and oracle disagree ({POLICY_NAMES[pol]})"
+
+    # configs[0]: n = 8 at t = 0, M = 32; 512 seeded instances in one batch
+    tr = T.concat([T.config1(i) for i in range(512)], "cfg1x512", 32, 2, 8)
+    ms, outs = gpu_run(tr, list(POLICIES))
+    orc = None
+    if svf_ref:
+        oms = [_oracle_ms(svf_ref, tr, p, 1) for p in POLICIES]
+        for p, (_, r) in zip(POLICIES, oms):
+            check("configs[0]", p, outs[p], r)
+        orc = {"ms_1_core": sum(m for m, _ in oms), "cores": 1, "sample": "the same 512 instances x 4 policies"}
+    entry("configs[0] tiny offline instance, 512 seeds", tr, list(POLICIES), ms, outs, orc)
+
+    # configs[1]: one online trace, n = 2,000
+    tr = T.config2(0)
+    for p in POLICIES:
+        ms, outs = gpu_run(tr, [p])
+        orc = None
+        if svf_ref:
+            oms, r = _oracle_ms(svf_ref, tr, p, 1)
+            check("configs[1]", p, outs[0], r)
+            orc = {"ms_1_core": oms, "cores": 1, "sample": "the same trace"}
+        e = entry("configs[1] single online trace n=2000", tr, [p], ms, outs, orc)
+        e["p99_latency"] = int(outs[0].p99_latency[0].item())
+
+    # configs[2]: 4,096 x 1,000 at rates 2, 4, 8: four policies per call
+    for lam in (2.0, 4.0, 8.0):
+        tr = T.config3(n_instances=args.instances, n=args.requests, lam=lam)
+        ms, outs = gpu_run(tr, list(POLICIES))
+        orc = None
+        if svf_ref:
+            t0 = time.perf_counter()
+            refs = [svf_ref.simulate(tr, p, n_threads=threads) for p in POLICIES]
+            all_ms = 1e3 * (time.perf_counter() - t0)
+            for p, r in zip(POLICIES, refs):
+                check(f"configs[2] rate {lam:g}", p, outs[p], r)
+            sub = tr.subset(range(0, tr.n_instances, max(1, tr.n_instances // 64)))
+            one_ms = sum(_oracle_ms(svf_ref, sub, p, 1)[0] for p in POLICIES)
+            orc = {"ms_all_cores": all_ms, "cores": threads, "sample": "the same batch x 4 policies",
+                   "ms_1_core_scaled": one_ms * tr.n_instances / sub.n_instances,
+                   "one_core_sample": f"{sub.n_instances} of {tr.n_instances} instances x 4 policies, scaled by the instance count"}
+        entry(f"configs[2] batched simulation, Poisson rate {lam:g}", tr, list(POLICIES), ms, outs, orc)
+
+    # configs[3]: one instance of 200,000 requests: a single serial step chain
+    tr = T.config4()
+    refs4 = None
+    if svf_ref:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(len(POLICIES)) as ex:          # each policy alone on one core, side by side
+            refs4 = list(ex.map(lambda p: _oracle_ms(svf_ref, tr, p, 1), POLICIES))
+    for p in POLICIES:
+        ms, outs = gpu_run(tr, [p])
+        orc = None
+        if refs4:
+            check("configs[3]", p, outs[0], refs4[p][1])
+            orc = {"ms_1_core": refs4[p][0], "cores": 1, "sample": "the same trace (the four policies timed side by side, one core each)"}
+        entry("configs[3] high-concurrency single instance n=200000", tr, [p], ms, outs, orc)
+
+    # configs[4]: 256 x 5,000, bimodal outputs: the (M, p) grid under SVF, 1-bit SVF, SJF
+    pols5 = [B.SVF, B.SVF_1BIT, B.SJF]
+    for M in (50_000, 200_000, 800_000):
+        for pf in (0.0, 0.05, 0.2):
+            tr = T.config5(M=M, p_flip=pf)
+            ms, outs = gpu_run(tr, pols5)
+            orc = None
+            if svf_ref:
+                t0 = time.perf_counter()
+                refs = [svf_ref.simulate(tr, p, n_threads=threads) for p in pols5]
+                all_ms = 1e3 * (time.perf_counter() - t0)
+                for p, o_, r in zip(pols5, outs, refs):
+                    check(f"configs[4] M={M} p={pf:g}", p, o_, r)
+                orc = {"ms_all_cores": all_ms, "cores": threads, "sample": "the same batch x 3 policies"}
+                if pf == 0.0:
+                    sub = tr.subset(range(0, tr.n_instances, 32))
+                    one_ms = sum(_oracle_ms(svf_ref, sub, p, 1)[0] for p in pols5)
+                    orc["ms_1_core_scaled"] = one_ms * tr.n_instances / sub.n_instances
+                    orc["one_core_sample"] = f"{sub.n_instances} of {tr.n_instances} instances x 3 policies, scaled by the instance count"
+            entry(f"configs[4] 1-bit SVF sweep M={M} p={pf:g}", tr, pols5, ms, outs, orc)
+    return info
 
 
 def bound_extras(B, torch, dev, args):
@@ -478,7 +634,7 @@ def cpu_baseline(args):
     from oracle import svf_ref
     svf_ref.build()
     threads = min(os.cpu_count() or 1, svf_ref.max_threads())
-    n_inst = min(args.instances, 2048)
+    n_inst = args.instances
     sample = T.config3(n_instances=n_inst, n=args.requests, lam=args.lam)
     oracle_step(svf_ref, sample.subset(range(min(8, n_inst))), threads)
     t0 = time.perf_counter()
@@ -490,8 +646,9 @@ def cpu_baseline(args):
             break
     dt = time.perf_counter() - t0
     return {"value": sample.request_steps * len(POLICIES) * reps / dt, "unit": UNIT, "cores": threads,
-            "kind": "oracle", "sample": f"{n_inst} of {args.instances} instances x {args.requests} requests x 4 policies, "
-                                        f"{reps} repetitions, {dt:.1f} s, instance-parallel over {threads} host threads"}
+            "kind": "oracle", "nproc": os.cpu_count(),
+            "sample": f"all {n_inst} instances x {args.requests} requests x 4 policies (rank 0's batch), "
+                      f"{reps} repetitions, {dt:.1f} s, instance-parallel over {threads} host threads"}
 
 
 def main():

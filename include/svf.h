@@ -195,6 +195,10 @@ int64_t svf_last_launch_count(int which);
 void svf_set_profiling(int mode);
 int svf_simulate_phase_ms(float* ms_out);
 int svf_simulate_work_counts(uint64_t* counts_out);
+/* The same for svf_admit (profiling mode 1 or 2): ms_out ([host] float[4]): [0] a1 + a2 keys, packing
+ * and validation, [1] a3 the sorts, [2] a4 + a5 the admission kernels (and the copy of the sorted
+ * words, if asked for), [3] the whole call. */
+int svf_admit_phase_ms(float* ms_out);
 
 const char* svf_status_string(int status);
 const char* svf_version(void);

@@ -25,7 +25,7 @@ EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_w
            "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies",
            "svf_volume_lower_bound_workspace_bytes", "svf_volume_lower_bound", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
            "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
-           "svf_simulate_work_counts")
+           "svf_simulate_work_counts", "svf_admit_phase_ms")
 
 
 class SvfError(RuntimeError):
@@ -99,6 +99,8 @@ def lib():
         L.svf_simulate_phase_ms.argtypes = [C.POINTER(C.c_float)]
         L.svf_simulate_work_counts.restype = C.c_int
         L.svf_simulate_work_counts.argtypes = [C.POINTER(C.c_uint64)]
+        L.svf_admit_phase_ms.restype = C.c_int
+        L.svf_admit_phase_ms.argtypes = [C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -129,6 +131,13 @@ def simulate_phase_ms():
     """(phase A, phase B, phase C, whole call) in ms for the last profiled svf_simulate call."""
     buf = (C.c_float * 4)()
     _check(lib().svf_simulate_phase_ms(buf), "svf_simulate_phase_ms")
+    return tuple(float(x) for x in buf)
+
+
+def admit_phase_ms():
+    """(keys + validation, sorts, admission, whole call) in ms for the last profiled svf_admit call."""
+    buf = (C.c_float * 4)()
+    _check(lib().svf_admit_phase_ms(buf), "svf_admit_phase_ms")
     return tuple(float(x) for x in buf)
 
 

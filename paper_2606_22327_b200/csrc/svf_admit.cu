@@ -455,6 +455,17 @@ void admit_ws_layout(AdmitWs* w, char* base, int64_t n_wait, int64_t n_run)
 }
 
 thread_local int64_t g_launches_admit = 0;
+thread_local bool g_admit_events_valid = false;
+thread_local cudaEvent_t g_admit_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+
+void admit_mark(int i, cudaStream_t st)
+{
+    if (!profiling_mode()) return;
+    if (!g_admit_ev[0])
+        for (int k = 0; k < 4; ++k) cudaEventCreate(&g_admit_ev[k]);
+    cudaEventRecord(g_admit_ev[i], st);
+    if (i == 3) g_admit_events_valid = true;
+}
 
 }  // namespace
 
@@ -494,6 +505,8 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return SVF_ECUDA;
     cudaStream_t st = (cudaStream_t)stream;
 
+    g_admit_events_valid = false;
+    admit_mark(0, st);
     k_admit_init<<<1, 1, 0, st>>>(w.flags);
     ++g_launches_admit;
     // a1 + a2
@@ -507,12 +520,14 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
         k_admit_validate<<<(unsigned)blocks, 256, 0, st>>>(n_wait, w_s, w_o, w_a, n_run, r_kv, r_rem, w.r0, w.flags);
         ++g_launches_admit;
     }
+    admit_mark(1, st);
     // a3: the waiting queue in priority order; the running set by finish time
     rc = sort_u64(w.wsort, w.w0, w.w1, w.w0, n_wait, 32, 64, st, &g_launches_admit);
     if (rc) return SVF_ECUDA;
     // a4 + a5: the maximal feasible prefix by bisection on one CTA; it also orders the running set
     // (for the serial kernels, should they be needed), so the device-wide sort of it is skipped
     const bool prefix = n_run <= AP_RUN_MAX;
+    if (prefix) admit_mark(2, st);            // (else the running set's device-wide sort still belongs to phase 1)
     if (prefix) {
         if (cudaFuncSetAttribute(k_admit_prefix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
         k_admit_prefix<<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
@@ -521,6 +536,7 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     } else {
         rc = sort_u64(w.rsort, w.r0, w.r1, w.r0, n_run, 32, 64, st, &g_launches_admit);
         if (rc) return SVF_ECUDA;
+        admit_mark(2, st);
     }
     const uint64_t* rdirect = prefix ? w.r1 : nullptr;
     const int* fast = prefix ? w.fast : nullptr;
@@ -538,5 +554,17 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
         rc = sort_result_to(w.wsort, sorted_words_out, n_wait, st, &g_launches_admit);
         if (rc) return SVF_ECUDA;
     }
+    admit_mark(3, st);
     return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
+}
+
+extern "C" int svf_admit_phase_ms(float* ms_out)
+{
+    if (!ms_out || !g_admit_events_valid) return SVF_EINVAL;
+    if (cudaEventSynchronize(g_admit_ev[3]) != cudaSuccess) return SVF_ECUDA;
+    cudaEventElapsedTime(&ms_out[0], g_admit_ev[0], g_admit_ev[1]);
+    cudaEventElapsedTime(&ms_out[1], g_admit_ev[1], g_admit_ev[2]);
+    cudaEventElapsedTime(&ms_out[2], g_admit_ev[2], g_admit_ev[3]);
+    cudaEventElapsedTime(&ms_out[3], g_admit_ev[0], g_admit_ev[3]);
+    return SVF_OK;
 }

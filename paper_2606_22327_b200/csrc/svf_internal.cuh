@@ -116,6 +116,7 @@ int keys_launch(int policy, int64_t n, const int32_t* s, const int32_t* o, const
                 const uint8_t* bit, int32_t O0, int32_t O1, uint64_t* words, int32_t* status,
                 cudaStream_t st, int64_t* launches);
 
-int sm_count();   // SMs of the current device (cached)
+int sm_count();   // SMs of the current device (asked every time; 148 without a device)
+int profiling_mode();   // svf_set_profiling's switch of this host thread (svf_simulate.cu)
 
 }  // namespace svf

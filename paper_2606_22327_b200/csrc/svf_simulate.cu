@@ -551,6 +551,7 @@ void prof_mark(int i, cudaStream_t st)
 }  // namespace
 
 int64_t sim_last_launches() { return g_launches_sim; }
+int profiling_mode() { return g_profiling; }
 
 }  // namespace svf
 

@@ -153,6 +153,47 @@ class Trace:
         return int(h)
 
 
+def fnv1a64(data: bytes) -> int:
+    """FNV-1a, 64 bit, over a byte string (offset basis 0xcbf29ce484222325, prime 0x100000001b3)."""
+    h = 0xCBF29CE484222325
+    for b in data:
+        h = ((h ^ b) * 0x100000001B3) & 0xFFFFFFFFFFFFFFFF
+    return h
+
+
+def trace_fingerprint(tr: "Trace") -> str:
+    """The identity of a config's input arrays as printed by bench.py: FNV-1a-64 (hex) over the
+    little-endian bytes of (I, N, M, O0, O1, Trace.checksum()) -- the checksum folds every element of
+    offsets / arrival / prompt / output / bit with its position, so the 48 bytes pin all of them.
+    (FNV itself is sequential byte by byte: the large arrays go through the vectorised fold first.)"""
+    words = np.array([tr.n_instances, tr.n_requests, tr.M, tr.O0, tr.O1], dtype=np.int64).view(np.uint64)
+    words = np.concatenate([words, np.array([tr.checksum()], dtype=np.uint64)])
+    return f"{fnv1a64(words.astype('<u8').tobytes()):016x}"
+
+
+def admit_state(seed: int, n_wait: int, n_run: int, M: int, fill: float = 0.8):
+    """Inputs of one stateless admission decision (bench.py's svf_admit sweep; BASELINE.json configs[3]
+    laws for the waiting queue): waiting (s, o, a, bit) in arrival order and a running set (kv, rem)
+    whose remaining steps are uniform and whose held tokens are scaled so that the set alone peaks
+    at ``fill * M`` -- a loaded engine with room for a few more.  Input shaping only: sorting and
+    running sums of the generator's own draws, none of the method's decisions."""
+    sd = instance_seed(88, seed)
+    w_s = lognormal_int(sd, 2, 3, n_wait, 1000.0, 0.8, 16, 8192)
+    w_o = lognormal_int(sd, 4, 5, n_wait, 400.0, 1.0, 1, 4096)
+    w_a = np.sort(uniform_int(sd, 1, n_wait, 0, 5000))
+    w_bit = (w_o > 400).astype(np.uint8)
+    rem_hi = int(max(8, min(3000, 1.6 * M / max(n_run, 1))))
+    r_rem = uniform_int(sd, 6, n_run, 1, rem_hi)
+    r_kv = lognormal_int(sd, 7, 8, n_run, 1200.0, 0.8, 16, 12000)
+    if n_run:
+        order = np.argsort(-r_rem, kind="stable")
+        cum = np.cumsum(r_kv[order].astype(np.int64)).astype(np.float64)
+        growth = (r_rem[order].astype(np.int64) * np.arange(1, n_run + 1)).astype(np.float64)
+        scale = float(np.clip(((fill * M - growth) / cum).min(), 0.0, 1.0))
+        r_kv = np.maximum((r_kv * scale).astype(np.int32), 0)
+    return w_s, w_o, w_a, w_bit, r_kv, r_rem
+
+
 def concat(parts, name, M, O0, O1, meta=None) -> Trace:
     sizes = [p.n_requests for p in parts]
     offsets = np.zeros(len(parts) + 1, dtype=np.int64)
