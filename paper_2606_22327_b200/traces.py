@@ -346,17 +346,24 @@ def geometric_int(seed: int, stream: int, n: int, mu: float, hi: int) -> np.ndar
     return np.clip(k, 1, hi).astype(np.int32)
 
 
+def onebit_proxies(mu: float, theta: int):
+    """Thm 3.5's proxy lengths for threshold theta under Geo(mu), rounded to integers >= 1
+    (reading R9): O0 = 1/mu - theta q^theta / (1 - q^theta) (short: o <= theta), O1 = theta + 1/mu (long)."""
+    q_t = (1.0 - mu) ** theta
+    O0 = max(1, int(round(1.0 / mu - theta * q_t / (1.0 - q_t))))
+    O1 = max(1, int(round(theta + 1.0 / mu)))
+    return O0, O1
+
+
 def stochastic(n_instances: int = 64, n: int = 1000, lam: float = 1.0, mean_o: float = 293.0,
-               o_hi: int = 4096, M: int = 300_000, first_instance: int = 0) -> Trace:
+               o_hi: int = 4096, M: int = 300_000, first_instance: int = 0, theta: int = None) -> Trace:
     """Poisson(lam) arrivals, o ~ Geo(1/mean_o) truncated at o_hi (mean 293 and budget 4,096 are the
     paper's calibration, PAPER.md:870), prompts as config 2.  1-bit constants follow Thm 3.5's
     conditional-expectation recipe at theta = mean_o, rounded to integers:
     O0 = 1/mu - theta q^theta / (1 - q^theta), O1 = theta + 1/mu, q = 1 - mu."""
     mu = 1.0 / mean_o
-    theta = int(round(mean_o))
-    q_t = (1.0 - mu) ** theta
-    O0 = max(1, int(round(1.0 / mu - theta * q_t / (1.0 - q_t))))
-    O1 = max(1, int(round(theta + 1.0 / mu)))
+    theta = int(round(mean_o)) if theta is None else int(theta)      # the 1-bit threshold: bit = (o > theta)
+    O0, O1 = onebit_proxies(mu, theta)
     parts = []
     for j in range(first_instance, first_instance + n_instances):
         sd = instance_seed(6, j, variant=int(round(lam * 16)))
@@ -364,4 +371,5 @@ def stochastic(n_instances: int = 64, n: int = 1000, lam: float = 1.0, mean_o: f
         s = lognormal_int(sd, _ST_S1, _ST_S2, n, 600.0, 0.8, 16, 4096)
         o = geometric_int(sd, _ST_O1, n, mu, o_hi)
         parts.append(_one("", a, s, o, (o > theta).astype(np.uint8), M, O0, O1))
-    return concat(parts, f"geo[lam={lam:g},1/mu={mean_o:g}]", M, O0, O1, {"config": 6, "lam": lam, "mu": mu})
+    return concat(parts, f"geo[lam={lam:g},1/mu={mean_o:g},theta={theta}]", M, O0, O1,
+                  {"config": 6, "lam": lam, "mu": mu, "theta": theta})

@@ -180,3 +180,29 @@ def test_report_layer_on_cuda_tensors(B, oracle):
     for k in ("mean_per_token_latency", "p95_per_token_latency", "token_throughput"):
         assert abs(got[k] - want[k]) <= 1e-12 * max(1.0, abs(want[k])), k
         assert abs(cpu[k] - want[k]) <= 1e-12 * max(1.0, abs(want[k])), k
+
+
+def test_stochastic_regime_report(B, oracle):
+    """NEXT-3: on the App. H reference workload the GPU's estimate of E[TEL] per request, over Lemma
+    H.1's lower bound on OPT (Eq. 89), sits below the bounds of Thm 3.4 (SVF) and Thm 3.5 (1-bit SVF) and
+    not below 1 by more than sampling noise; the estimate itself equals the oracle's (integers in, one
+    division)."""
+    import torch
+    from paper_2606_22327_b200 import report as R
+    mu, M, p_max = 1.0 / 293.0, 300_000, 8192
+    for rho, theta in ((0.6, 293), (0.9, 147)):
+        probe = T.stochastic(n_instances=48, n=800, lam=1.0, M=M)
+        mean_s = float(probe.prompt.mean())
+        lam = R.rate_for_load(rho, mu, mean_s, M, p_max)
+        tr = T.stochastic(n_instances=48, n=800, lam=lam, M=M, theta=theta)
+        c = R.stochastic_constants(mu, mean_s, lam, M, p_max, theta=theta)
+        assert abs(c["rho"] - rho) < 1e-9 and (tr.O0, tr.O1) == T.onebit_proxies(mu, theta)
+        dt = B.DeviceTrace.from_host(tr)
+        outs = B.svf_simulate_policies(dt, [B.SVF, B.SVF_1BIT], want=("total_latency", "status"))
+        torch.cuda.synchronize()
+        for pol, out, bound in ((B.SVF, outs[0], c["thm34_bound"]), (B.SVF_1BIT, outs[1], c["thm35_bound"])):
+            est = R.mean_request_latency(out.total_latency, dt.offsets, out.status)
+            ref = oracle.simulate(tr, pol, n_threads=8)
+            assert est == float(ref.total_latency.sum()) / tr.n_requests
+            ratio = est / c["opt_lower_bound"]
+            assert 0.9 < ratio <= bound, (rho, theta, pol, ratio, bound)

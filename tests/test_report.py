@@ -87,3 +87,41 @@ def test_paper_metrics_over_two_ranks(oracle):
     assert got["requests"] == want["requests"]
     for k in ("mean_per_token_latency", "p95_per_token_latency", "token_throughput"):
         assert abs(got[k] - want[k]) <= 1e-12 * max(1.0, abs(want[k])), k
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: the constants of the stochastic analysis (PAPER.md 3.4, App. H) by hand values
+# ---------------------------------------------------------------------------------------------
+def test_stochastic_constants_hand_values():
+    """mu = 1/2, theta = 2, E[s] = 3, lambda = 1, M = 100, p_max = 20 (alpha = 0.2), worked by hand:
+    q^theta = 1/4, d = 2 (1/4) / (3/4) = 2/3, eps = d^2/2 = 2/9, O0 = 2 - 2/3 = 4/3, O1 = 2 + 2 = 4;
+    E[vol] = 3*2 + 4 = 10 (Eq. 101); rho = 10 / (0.8 * 50) = 1/4; Thm 3.4: 1 + 2 / (0.8 * 0.5 * 0.75) = 23/3;
+    Thm 3.5: 1 + 10 / (10 - 2/9) * 20/3 = 1 + (45/44)(20/3) = 86/11; W_exact = 1 * (1/2)/(1/4) * (3 + 4) = 14
+    (Eq. 89), OPT >= max{2, 14/100} = 2."""
+    c = R.stochastic_constants(mu=0.5, mean_s=3.0, lam=1.0, M=100.0, p_max=20.0, theta=2)
+    want = {"alpha": 0.2, "E_vol": 10.0, "rho": 0.25, "thm34_bound": 23.0 / 3.0, "W_exact": 14.0, "opt_lower_bound": 2.0,
+            "eps": 2.0 / 9.0, "O0": 4.0 / 3.0, "O1": 4.0, "thm35_bound": 86.0 / 11.0}
+    for k, v in want.items():
+        assert abs(c[k] - v) < 1e-12 * max(1.0, abs(v)), (k, c[k], v)
+    # O0 and O1 ARE the conditional means of Geo(1/2) split at theta = 2: (1/2 + 2/4) / (3/4) and 2 + 2
+    pk = np.array([0.5 ** k for k in range(1, 60)])
+    ks = np.arange(1, 60)
+    assert abs((pk[:2] * ks[:2]).sum() / pk[:2].sum() - c["O0"]) < 1e-12
+    assert abs((pk[2:] * ks[2:]).sum() / pk[2:].sum() - c["O1"]) < 1e-9
+    # the queueing term takes over under load: lambda = 20 -> W_exact / M = 2.8 > 1/mu; rho >= 1 -> no bound
+    assert abs(R.stochastic_constants(0.5, 3.0, 20.0, 100.0, 20.0)["opt_lower_bound"] - 2.8) < 1e-12
+    assert R.stochastic_constants(0.5, 3.0, 20.0, 100.0, 20.0)["thm34_bound"] == float("inf")
+    # rate_for_load inverts rho; the printed proxies of the App. H calibration (1/mu = theta = 293): 123, 586
+    lam = R.rate_for_load(0.6, 1.0 / 293.0, 597.0, 300_000.0, 8192.0)
+    assert abs(R.stochastic_constants(1.0 / 293.0, 597.0, lam, 300_000.0, 8192.0)["rho"] - 0.6) < 1e-12
+    assert T.onebit_proxies(1.0 / 293.0, 293) == (123, 586)
+    # eps decays as theta grows (the Remark, PAPER.md:197)
+    eps = [R.stochastic_constants(1.0 / 293.0, 597.0, lam, 300_000.0, 8192.0, theta=th)["eps"] for th in (64, 147, 293, 586, 1172)]
+    assert all(a > b for a, b in zip(eps[1:], eps[2:])) and eps[-1] < 0.02 * eps[1]
+
+
+def test_mean_request_latency_is_total_over_requests():
+    off = torch.tensor([0, 3, 3, 10], dtype=torch.int64)
+    tel = torch.tensor([30, 0, 140], dtype=torch.int64)
+    assert R.mean_request_latency(tel, off) == 17.0
+    assert R.mean_request_latency(tel, off, torch.tensor([0, 0, 19], dtype=torch.int32)) == 10.0
