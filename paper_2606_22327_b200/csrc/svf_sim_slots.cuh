@@ -145,6 +145,7 @@ struct SlotArgs {
     const uint32_t* layout_bad;      // one word: the offsets of the call are not monotone (k_sim_check_layout)
     unsigned long long* work_counts; // [4] E, U, evaluations, blocked evaluations (COUNT variant only)
     char* gstate; size_t slot_bytes; // per-CTA state when it does not fit in shared memory
+    int ext_global;                  // bitmaps in shared memory, ext slots in the per-CTA global slot
     int ecap;                        // ext slots per instance
     int qcap;                        // bitmap capacity (ranks)
 };
@@ -353,7 +354,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
     const int capL0 = QREG ? 0 : (g.qcap + 31) / 32, capL1 = (capL0 + 31) / 32;
     uint32_t* L0 = reinterpret_cast<uint32_t*>(sbase);
     uint32_t* L1 = reinterpret_cast<uint32_t*>(sbase + align_up((size_t)capL0 * 4, 16));
-    char* ebase = reinterpret_cast<char*>(L1) + align_up((size_t)capL1 * 4, 16);
+    char* ebase = (QREG || !g.ext_global) ? reinterpret_cast<char*>(L1) + align_up((size_t)capL1 * 4, 16)
+                                          : g.gstate + (size_t)blockIdx.x * g.slot_bytes;
     const size_t estride = align_up((size_t)g.ecap * 4, 16);
     int32_t* ef = reinterpret_cast<int32_t*>(ebase);
     uint32_t* eB = reinterpret_cast<uint32_t*>(ebase + estride);

@@ -368,6 +368,7 @@ struct SimConfig {
     bool slots;             // register-resident kernel (M < 2^30); else the wide sorted-array kernel
     int ecap, qcap;         // slots kernel: ext slots per instance, bitmap capacity
     bool qreg;              // slots kernel: waiting bitmap in one register per lane (<= 1024 ranks)
+    bool ext_global;        // slots kernel, one warp per item: bitmaps in shared memory, ext slots in a global slot
     size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
     size_t gslot_bytes;     // bytes of the per-CTA slot in global memory (0: none)
     int max_cta_per_sm;     // bound on resident CTAs per SM (sizes the global slots)
@@ -393,7 +394,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.sort_hi = c.sb + 32 + c.ib;
     c.cap = (int)((mx + 31) / 32 * 32);
     c.slots = M < ((int64_t)1 << 30);
-    c.ecap = 0; c.qcap = c.cap; c.qreg = false;
+    c.ecap = 0; c.qcap = c.cap; c.qreg = false; c.ext_global = false;
     // group width.  Register-slot kernels: one WARP per item (512 register slots) unless the running
     // set can outgrow them and there are warps to spare: R is at most mx and, at a few hundred
     // tokens per running request, about M / 512.  Measured: a CTA-wide group is slower than a warp
@@ -405,7 +406,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     int threads = 32;
     if (c.slots) {
         const int64_t r_est = mx < M / 512 ? mx : M / 512;
-        if (r_est > 32 * SLOT_K && w >= 4) threads = 128;
+        if (r_est > 32 * SLOT_K && w >= 2) threads = 128;
         if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
     } else {
         while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
@@ -422,6 +423,16 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
             c.ecap = ext_of(32);
             c.state_bytes = QREG_SMEM_BYTES;
             c.smem = true;
+            c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
+            c.max_cta_per_sm = 32;
+        } else if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT &&
+                   slot_state_bytes(c.qcap, 0) <= SMEM_WARP_STATE_LIMIT) {
+            // one warp per item, more than 1024 requests per instance: the bitmaps stay in shared
+            // memory, the ext slots (only touched when more than 512 requests run at once, which the
+            // choice of the group width above makes unlikely) go to a global slot per CTA
+            c.ecap = ext_of(32);
+            c.state_bytes = slot_state_bytes(c.qcap, 0);
+            c.smem = true; c.ext_global = true;
             c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
             c.max_cta_per_sm = 32;
         } else {
@@ -563,9 +574,10 @@ namespace {
 size_t sim_workspace_bytes(const svf_trace_t* tr, int P)
 {
     if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0 || P < 1 || P > MAX_POLICIES) return 0;
-    // M is not known here: size for the larger of the two kernels' layouts
+    // M is not known here and picks the kernel family (through min(max_instance, M / 512) against the
+    // register-slot capacities 512 and 2048, and through M >= 2^30): size for the largest layout
     size_t need = 0;
-    for (int64_t M : {(int64_t)0, (int64_t)1 << 30}) {
+    for (int64_t M : {(int64_t)0, (int64_t)512 * 600, (int64_t)512 * 3000, (int64_t)1 << 30}) {
         SimConfig c = sim_config(tr, M, P);
         SimWs w;
         int64_t slots = c.gslot_bytes ? (int64_t)c.max_cta_per_sm * sm_count() : 0;
@@ -725,7 +737,7 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
 
     // ---- phase B: one persistent launch over P x I work items -------------------------------------
     q.work_ctr = w.work_ctr; q.work_counts = w.counts; q.layout_bad = w.layout_bad;
-    q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap;
+    q.gstate = w.gstate; q.slot_bytes = w.slot_bytes; q.ecap = c.ecap; q.qcap = c.qcap; q.ext_global = c.ext_global ? 1 : 0;
     const bool count = g_profiling == 2;
     if (count) {
         if (cudaMemsetAsync(w.counts, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
