@@ -34,23 +34,34 @@ __device__ __forceinline__ uint32_t digit_of(uint64_t w, int shift, uint32_t mas
     return (uint32_t)(w >> shift) & mask;
 }
 
-// lanes of the warp holding the same digit (9 bits: SORT_RADIX marks an invalid lane), by one
-// ballot per bit: no MATCH instruction on the critical path
+// lanes of the warp holding the same digit, by one ballot per digit bit (no MATCH instruction on
+// the critical path: measured slower).  Four instructions per bit, written out in PTX because the
+// compiler's own form of `peers &= bit ? m : ~m` took six to seven (extract, ISETP, VOTE, NOT, SEL,
+// AND): test the bit into a predicate (one LOP3), ballot, complement the ballot where the own bit
+// is clear (predicated), and it in.  An invalid lane (past the end of a ragged tile) matches the
+// other invalid lanes only.
 #ifndef SVF_SORT_USE_MATCH
 #define SVF_SORT_USE_MATCH 0
 #endif
+template <bool FULL>
 __device__ __forceinline__ uint32_t warp_match_digit(uint32_t d, bool valid)
 {
 #if SVF_SORT_USE_MATCH
-    return __match_any_sync(0xffffffffu, d);
+    return __match_any_sync(0xffffffffu, FULL ? d : (valid ? d : SORT_RADIX));
 #else
-    uint32_t peers = __ballot_sync(0xffffffffu, valid);
-    if (!valid) peers = ~peers;
+    uint32_t peers = 0xffffffffu;
+    if (!FULL) {
+        peers = __ballot_sync(0xffffffffu, valid);
+        if (!valid) peers = ~peers;
+    }
 #pragma unroll
     for (int b = 0; b < SORT_RADIX_BITS; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const uint32_t m = __ballot_sync(0xffffffffu, bit);
-        peers &= bit ? m : ~m;
+        asm("{\n\t.reg .pred p;\n\t.reg .b32 m, t;\n\t"
+            "and.b32 t, %1, %2;\n\t"
+            "setp.ne.u32 p, t, 0;\n\t"
+            "vote.sync.ballot.b32 m, p, 0xffffffff;\n\t"
+            "@!p not.b32 m, m;\n\t"
+            "and.b32 %0, %0, m;\n\t}" : "+r"(peers) : "r"(d), "r"(1u << b));
     }
     return peers;
 #endif
@@ -174,6 +185,139 @@ __device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gsrc, ui
 }
 
 // ---- one onesweep pass -----------------------------------------------------------------------
+struct PassSmem {
+    uint64_t* staging; uint32_t *whist, *thist, *toff_s, *gbase_s, *warp_tot;
+};
+
+// the body for one tile; FULL = the tile holds SORT_TILE words (every tile but the last): the
+// "is this element inside the tile" tests are compiled out of it
+template <bool FULL>
+__device__ __forceinline__ void sort_pass_tile(const PassSmem& sm, int tile_n, uint32_t tile,
+                                               int shift, uint32_t mask, uint32_t* __restrict__ status,
+                                               const uint32_t* __restrict__ bases, uint64_t* __restrict__ dst)
+{
+    constexpr int WARPS = SORT_THREADS / 32;
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    const int wbase = wrp * 32 * SORT_IPT;
+    // the digit of every key of this thread, once, four to a register; the keys themselves stay in
+    // the staged tile until the scatter (16 x 64 bit in registers through the ranking would spill)
+    uint32_t dig4[SORT_IPT / 4];
+#pragma unroll
+    for (int i = 0; i < SORT_IPT / 4; ++i) dig4[i] = 0;
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) dig4[i >> 2] |= digit_of(sm.staging[wbase + i * 32 + lane], shift, mask) << (8 * (i & 3));
+    auto dig = [&](int i) { return (dig4[i >> 2] >> (8 * (i & 3))) & 0xffu; };
+
+    // the tile's digit counts first (shared-memory atomics), published BEFORE the ranking: the
+    // successors' look-back then finds an aggregate while this tile is still ranking (deriving the
+    // counts from the ranking's warp histograms instead saves the atomics but publishes late: 2.11
+    // against 1.78 ms for the 2^26-word sort)
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i)
+        if (FULL || (wbase + i * 32 + lane) < tile_n) atomicAdd(&sm.thist[dig(i)], 1u);
+    __syncthreads();
+    const uint32_t count = sm.thist[tid];
+    volatile uint32_t* st = status + (size_t)tile * SORT_RADIX + tid;
+    *st = (tile == 0 ? FLAG_INCL : FLAG_AGG) | count;
+    {   // tile-level exclusive scan of the counts
+        uint32_t inc = count;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) sm.warp_tot[wrp] = inc;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < wrp; ++w) off += sm.warp_tot[w];
+        sm.toff_s[tid] = off + inc - count;
+    }
+
+    // per-warp stable ranking with digit ballots; two ranks (< 4096 each) to a register
+    uint32_t* wh = sm.whist + wrp * SORT_RADIX;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    uint32_t rank2[SORT_IPT / 2];
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        const bool valid = FULL || (wbase + i * 32 + lane) < tile_n;
+        const uint32_t d = dig(i);
+        const uint32_t peers = warp_match_digit<FULL>(d, valid);
+        // the highest peer owns the warp-private counter of its digit for this round
+        const int leader = 31 - __clz(peers);
+        uint32_t base = 0;
+        if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
+        base = __shfl_sync(0xffffffffu, base, leader);
+        __syncwarp();
+        const uint32_t r = base + __popc(peers & lt_mask);
+        if (i & 1) rank2[i >> 1] |= r << 16; else rank2[i >> 1] = r;
+    }
+    __syncthreads();
+
+    // digit d (thread d): exclusive scan of the warp-private counts over the warps; then the
+    // decoupled look-back over the predecessor tiles of this digit (their aggregates were
+    // published before their ranking, so this rarely waits)
+    {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) { uint32_t c = sm.whist[w * SORT_RADIX + tid]; sm.whist[w * SORT_RADIX + tid] = run; run += c; }
+        uint32_t excl = 0;
+        if (tile > 0) {
+            // eight predecessors per round trip to L2 (independent loads), consumed in order
+            constexpr int LOOK = 8;
+            int64_t look = (int64_t)tile - 1;
+            bool done = false;
+            while (!done) {
+                uint32_t v[LOOK];
+#pragma unroll
+                for (int q = 0; q < LOOK; ++q) {
+                    const int64_t idx = look - q;
+                    v[q] = idx >= 0 ? *(volatile uint32_t*)(status + (size_t)idx * SORT_RADIX + tid) : (2u << 30);   // past tile 0: an empty inclusive word
+                }
+                int used = 0;
+#pragma unroll
+                for (int q = 0; q < LOOK; ++q) {
+                    if (!done && used == q) {
+                        const uint32_t f = v[q] >> 30;
+                        if (f != 0) {
+                            excl += v[q] & VALUE_MASK;
+                            ++used;
+                            if (f == 2) done = true;
+                        }
+                    }
+                }
+                look -= used;
+            }
+            *st = FLAG_INCL | (excl + count);
+        }
+        sm.gbase_s[tid] = bases[tid] + excl - sm.toff_s[tid];    // modulo 2^32; dst index = gbase + slot
+    }
+    // every thread takes its keys out of the staged tile, then the tile is rewritten in digit order
+    uint64_t key[SORT_IPT];
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) key[i] = sm.staging[wbase + i * 32 + lane];
+    __syncthreads();
+
+    // scatter inside shared memory, then write coalesced runs
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) {
+        if (FULL || (wbase + i * 32 + lane) < tile_n) {
+            const uint32_t d = dig(i);
+            const uint32_t r = (i & 1) ? (rank2[i >> 1] >> 16) : (rank2[i >> 1] & 0xffffu);
+            sm.staging[sm.toff_s[d] + wh[d] + r] = key[i];
+        }
+    }
+    __syncthreads();
+    if (FULL) {
+#pragma unroll 4
+        for (int q = tid; q < SORT_TILE; q += SORT_THREADS) {
+            const uint64_t w = sm.staging[q];
+            dst[(uint32_t)(sm.gbase_s[digit_of(w, shift, mask)] + (uint32_t)q)] = w;
+        }
+    } else {
+        for (int q = tid; q < tile_n; q += SORT_THREADS) {
+            const uint64_t w = sm.staging[q];
+            dst[(uint32_t)(sm.gbase_s[digit_of(w, shift, mask)] + (uint32_t)q)] = w;
+        }
+    }
+}
+
 __global__ void __launch_bounds__(SORT_THREADS, 4) k_sort_pass(const SortPlan* __restrict__ plan,
                                                             int p, int64_t n, int shift,
                                                             uint32_t mask,
@@ -206,8 +350,6 @@ __global__ void __launch_bounds__(SORT_THREADS, 4) k_sort_pass(const SortPlan* _
 
     // stage the tile, then take it in warp-striped order: item i of lane l in warp w is element
     // w*32*IPT + i*32 + l of the tile (so ranks follow the input order = stability)
-    uint64_t key[SORT_IPT];
-    const int wbase = wrp * 32 * SORT_IPT;
     const bool bulk = (tile_n == SORT_TILE) && ((reinterpret_cast<uintptr_t>(src + tile_base) & 15u) == 0);
     if (bulk) {
         if (tid == 0) {
@@ -215,109 +357,15 @@ __global__ void __launch_bounds__(SORT_THREADS, 4) k_sort_pass(const SortPlan* _
             tma_load_1d(staging, src + tile_base, SORT_TILE * 8u, &bar);
         }
         mbar_wait(&bar, 0);
-#pragma unroll
-        for (int i = 0; i < SORT_IPT; ++i) key[i] = staging[wbase + i * 32 + lane];
     } else {
-#pragma unroll
-        for (int i = 0; i < SORT_IPT; ++i) {
-            int e = wbase + i * 32 + lane;
-            key[i] = e < tile_n ? __ldg(src + tile_base + e) : ~0ull;
-        }
-    }
-
-    // the tile's digit counts first (shared-memory atomics), published BEFORE the ranking: the
-    // successors' look-back then finds an aggregate while this tile is still ranking
-#pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i)
-        if ((wbase + i * 32 + lane) < tile_n) atomicAdd(&thist[digit_of(key[i], shift, mask)], 1u);
-    __syncthreads();
-    const uint32_t count = thist[tid];
-    volatile uint32_t* st = status + (size_t)tile * SORT_RADIX + tid;
-    *st = (tile == 0 ? FLAG_INCL : FLAG_AGG) | count;
-    {   // tile-level exclusive scan of the counts
-        uint32_t inc = count;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-        if (lane == 31) warp_tot[wrp] = inc;
+        // ragged or unaligned tile: plain coalesced loads into the same staging buffer
+        for (int e = tid; e < SORT_TILE; e += SORT_THREADS) staging[e] = e < tile_n ? __ldg(src + tile_base + e) : ~0ull;
         __syncthreads();
-        uint32_t off = 0;
-        for (int w = 0; w < wrp; ++w) off += warp_tot[w];
-        toff_s[tid] = off + inc - count;
     }
-
-    // per-warp stable ranking with digit ballots
-    uint32_t* wh = whist + wrp * SORT_RADIX;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    uint32_t rank[SORT_IPT];
-#pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
-        const bool valid = (wbase + i * 32 + lane) < tile_n;
-        const uint32_t d = valid ? digit_of(key[i], shift, mask) : SORT_RADIX;
-        const uint32_t peers = warp_match_digit(d, valid);
-        // the highest peer owns the warp-private counter of its digit for this round
-        const int leader = 31 - __clz(peers);
-        uint32_t base = 0;
-        if (valid && lane == leader) { base = wh[d]; wh[d] = base + __popc(peers); }
-        base = __shfl_sync(0xffffffffu, base, leader);
-        __syncwarp();
-        rank[i] = base + __popc(peers & lt_mask);
-    }
-    __syncthreads();
-
-    // digit d (thread d): exclusive scan of the warp-private counts over the warps; then the
-    // decoupled look-back over the predecessor tiles of this digit (their aggregates were
-    // published before their ranking, so this rarely waits)
-    {
-        uint32_t run = 0;
-#pragma unroll
-        for (int w = 0; w < WARPS; ++w) { uint32_t c = whist[w * SORT_RADIX + tid]; whist[w * SORT_RADIX + tid] = run; run += c; }
-        uint32_t excl = 0;
-        if (tile > 0) {
-            // eight predecessors per round trip to L2 (independent loads), consumed in order
-            constexpr int LOOK = 8;
-            int64_t look = (int64_t)tile - 1;
-            bool done = false;
-            while (!done) {
-                uint32_t v[LOOK];
-#pragma unroll
-                for (int q = 0; q < LOOK; ++q) {
-                    const int64_t idx = look - q;
-                    v[q] = idx >= 0 ? *(volatile uint32_t*)(status + (size_t)idx * SORT_RADIX + tid) : (2u << 30);   // past tile 0: an empty inclusive word
-                }
-                int used = 0;
-#pragma unroll
-                for (int q = 0; q < LOOK; ++q) {
-                    if (!done && used == q) {
-                        const uint32_t f = v[q] >> 30;
-                        if (f != 0) {
-                            excl += v[q] & VALUE_MASK;
-                            ++used;
-                            if (f == 2) done = true;
-                        }
-                    }
-                }
-                look -= used;
-            }
-            *st = FLAG_INCL | (excl + count);
-        }
-        gbase_s[tid] = bases[tid] + excl - toff_s[tid];    // modulo 2^32; dst index = gbase + slot
-    }
-    __syncthreads();
-
-    // scatter inside shared memory, then write coalesced runs
-#pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
-        if ((wbase + i * 32 + lane) < tile_n) {
-            uint32_t d = digit_of(key[i], shift, mask);
-            staging[toff_s[d] + wh[d] + rank[i]] = key[i];
-        }
-    }
-    __syncthreads();
-    for (int q = tid; q < tile_n; q += SORT_THREADS) {
-        uint64_t w = staging[q];
-        uint32_t d = digit_of(w, shift, mask);
-        dst[(uint32_t)(gbase_s[d] + (uint32_t)q)] = w;
-    }
+    (void)lane; (void)wrp;
+    PassSmem sm{staging, whist, thist, toff_s, gbase_s, warp_tot};
+    if (tile_n == SORT_TILE) sort_pass_tile<true>(sm, tile_n, tile, shift, mask, status, bases, dst);
+    else                     sort_pass_tile<false>(sm, tile_n, tile, shift, mask, status, bases, dst);
 }
 
 __global__ void k_sort_copy_result(const SortPlan* __restrict__ plan, uint64_t* __restrict__ out, int64_t n)
