@@ -85,30 +85,41 @@ __global__ void __launch_bounds__(512) k_sort_hist(const uint64_t* __restrict__ 
         mask[p] = (1u << wdt) - 1u;
     }
     // run-length accumulation: a digit that repeats costs one shared atomic per run, so the
-    // all-equal high digits of small keys do not serialise on a single bin
+    // all-equal high digits of small keys do not serialise on a single bin.  Branch free: the flush
+    // of a finished run is one PREDICATED atomic (a branch here diverges on every random digit and
+    // tripled the instruction count of this kernel)
     uint32_t last[NPASS], cnt[NPASS];
 #pragma unroll
     for (int p = 0; p < NPASS; ++p) { last[p] = 0; cnt[p] = 0; }
-
-    // four independent loads in flight per thread (the kernel is latency bound otherwise)
-    constexpr int UNR = 4;
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < n; i0 += stride * UNR) {
-        uint64_t w[UNR];
+    auto take = [&](uint64_t w) {
 #pragma unroll
-        for (int u = 0; u < UNR; ++u) { const int64_t i = i0 + u * stride; w[u] = i < n ? __ldg(in + i) : 0ull; }
-#pragma unroll
-        for (int u = 0; u < UNR; ++u) {
-            if (i0 + u * stride < n) {
-#pragma unroll
-                for (int p = 0; p < NPASS; ++p) {
-                    uint32_t d = digit_of(w[u], shift[p], mask[p]);
-                    if (d == last[p]) ++cnt[p];
-                    else { if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]); last[p] = d; cnt[p] = 1; }
-                }
-            }
+        for (int p = 0; p < NPASS; ++p) {
+            const uint32_t d = digit_of(w, shift[p], mask[p]);
+            const bool same = d == last[p];
+            if (!same && cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]);
+            cnt[p] = same ? cnt[p] + 1 : 1;
+            last[p] = d;
         }
+    };
+
+    // two words per 128-bit load, four loads in flight per thread; the tail (and an unaligned
+    // input) word by word
+    const bool vec = (reinterpret_cast<uintptr_t>(in) & 15u) == 0;
+    const int64_t n2 = vec ? (n >> 1) : 0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    constexpr int UNR = 4;
+    const ulonglong2* __restrict__ in2 = reinterpret_cast<const ulonglong2*>(in);
+    int64_t q0 = gid;
+    for (; q0 + (UNR - 1) * stride < n2; q0 += stride * UNR) {
+        ulonglong2 w[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) w[u] = __ldg(in2 + q0 + u * stride);
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) { take(w[u].x); take(w[u].y); }
     }
+    for (; q0 < n2; q0 += stride) { const ulonglong2 w = __ldg(in2 + q0); take(w.x); take(w.y); }
+    for (int64_t i = (n2 << 1) + gid; i < n; i += stride) take(__ldg(in + i));
 #pragma unroll
     for (int p = 0; p < NPASS; ++p) if (cnt[p]) atomicAdd(&sh[p * SORT_RADIX + last[p]], cnt[p]);
     __syncthreads();
@@ -254,7 +265,8 @@ __device__ __forceinline__ void sort_pass_tile(const PassSmem& sm, int tile_n, u
     // decoupled look-back over the predecessor tiles of this digit (their aggregates were
     // published before their ranking, so this rarely waits)
     {
-        uint32_t run = 0;
+        // (the digit's offset inside the tile is folded in: the scatter then needs one lookup per key)
+        uint32_t run = sm.toff_s[tid];
 #pragma unroll
         for (int w = 0; w < WARPS; ++w) { uint32_t c = sm.whist[w * SORT_RADIX + tid]; sm.whist[w * SORT_RADIX + tid] = run; run += c; }
         uint32_t excl = 0;
@@ -300,7 +312,7 @@ __device__ __forceinline__ void sort_pass_tile(const PassSmem& sm, int tile_n, u
         if (FULL || (wbase + i * 32 + lane) < tile_n) {
             const uint32_t d = dig(i);
             const uint32_t r = (i & 1) ? (rank2[i >> 1] >> 16) : (rank2[i >> 1] & 0xffffu);
-            sm.staging[sm.toff_s[d] + wh[d] + r] = key[i];
+            sm.staging[wh[d] + r] = key[i];
         }
     }
     __syncthreads();
