@@ -34,39 +34,6 @@ __device__ __forceinline__ uint32_t digit_of(uint64_t w, int shift, uint32_t mas
     return (uint32_t)(w >> shift) & mask;
 }
 
-// lanes of the warp holding the same digit, by one ballot per digit bit (no MATCH instruction on
-// the critical path: measured slower).  Four instructions per bit, written out in PTX because the
-// compiler's own form of `peers &= bit ? m : ~m` took six to seven (extract, ISETP, VOTE, NOT, SEL,
-// AND): test the bit into a predicate (one LOP3), ballot, complement the ballot where the own bit
-// is clear (predicated), and it in.  An invalid lane (past the end of a ragged tile) matches the
-// other invalid lanes only.
-#ifndef SVF_SORT_USE_MATCH
-#define SVF_SORT_USE_MATCH 0
-#endif
-template <bool FULL>
-__device__ __forceinline__ uint32_t warp_match_digit(uint32_t d, bool valid)
-{
-#if SVF_SORT_USE_MATCH
-    return __match_any_sync(0xffffffffu, FULL ? d : (valid ? d : SORT_RADIX));
-#else
-    uint32_t peers = 0xffffffffu;
-    if (!FULL) {
-        peers = __ballot_sync(0xffffffffu, valid);
-        if (!valid) peers = ~peers;
-    }
-#pragma unroll
-    for (int b = 0; b < SORT_RADIX_BITS; ++b) {
-        asm("{\n\t.reg .pred p;\n\t.reg .b32 m, t;\n\t"
-            "and.b32 t, %1, %2;\n\t"
-            "setp.ne.u32 p, t, 0;\n\t"
-            "vote.sync.ballot.b32 m, p, 0xffffffff;\n\t"
-            "@!p not.b32 m, m;\n\t"
-            "and.b32 %0, %0, m;\n\t}" : "+r"(peers) : "r"(d), "r"(1u << b));
-    }
-    return peers;
-#endif
-}
-
 // ---- histogram of every digit in one read of the input ---------------------------------------
 template <int NPASS>
 __global__ void __launch_bounds__(512) k_sort_hist(const uint64_t* __restrict__ in, int64_t n,
@@ -399,10 +366,10 @@ __global__ void k_sort_plan_identity(SortPlan* plan, const uint64_t* in) { plan-
 // rank[] (rank of id) and, if wanted, the (s, o, id, a) records in priority order.  HBM traffic:
 // 12-13 B read + 8 B (24 B with records) written per request, against 8 + 16 B per executed pass
 // of the device-wide sort.
-template <int IPT>
+template <int SORT_THREADS, int IPT>
 __global__ void __launch_bounds__(SORT_THREADS) k_seg_sort(SegSortArgs A)
 {
-    static_assert(SORT_THREADS == SORT_RADIX, "one thread per digit in the scans");
+    static_assert(SORT_THREADS == 128 || SORT_THREADS == 256, "seg_pass: one or two digits per thread in the scans");
     constexpr int WARPS = SORT_THREADS / 32;
     extern __shared__ __align__(16) uint64_t seg_buf[];       // [2][cap]
     __shared__ uint32_t whist[WARPS * SORT_RADIX];
@@ -558,21 +525,23 @@ int seg_sort_keys(const SegSortArgs& A, int64_t max_instance, cudaStream_t st, i
     B.cap = (int)((max_instance > 0 ? max_instance : 1) + 1) / 2 * 2;
     const size_t smem = (size_t)2 * B.cap * sizeof(uint64_t);
     // items per thread sized to the largest instance (registers: occupancy of small segments)
-#define SVF_SEG_LAUNCH(IPT)                                                                             \
+#define SVF_SEG_LAUNCH(T, IPT)                                                                          \
     do {                                                                                                \
-        cudaFuncSetAttribute(k_seg_sort<IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+        cudaFuncSetAttribute(k_seg_sort<T, IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
                              2 * SEG_SORT_MAX * (int)sizeof(uint64_t));   /* per device: set every time */ \
         int per_sm = 0;                                                                                 \
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort<IPT>, SORT_THREADS, smem) \
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_seg_sort<T, IPT>, T, smem)         \
                 != cudaSuccess || per_sm < 1)                                                           \
             per_sm = 1;                                                                                 \
         int64_t grid = (int64_t)per_sm * sm_count();                                                    \
         if (grid > B.I) grid = B.I;                                                                     \
-        k_seg_sort<IPT><<<(unsigned)grid, SORT_THREADS, smem, st>>>(B);                                 \
+        k_seg_sort<T, IPT><<<(unsigned)grid, T, smem, st>>>(B);                                         \
     } while (0)
-    if (B.cap <= 4 * SORT_THREADS) SVF_SEG_LAUNCH(4);
-    else if (B.cap <= 8 * SORT_THREADS) SVF_SEG_LAUNCH(8);
-    else SVF_SEG_LAUNCH(16);
+    // instances of at most 1024 requests: CTAs of four warps (half the per-pass overhead of the
+    // histogram reset and the digit scans, barriers over four warps, twice the CTAs per SM)
+    if (B.cap <= 8 * 128) SVF_SEG_LAUNCH(128, 8);
+    else if (B.cap <= 8 * 256) SVF_SEG_LAUNCH(256, 8);
+    else SVF_SEG_LAUNCH(256, 16);
 #undef SVF_SEG_LAUNCH
     ++*launches;
     return (int)cudaGetLastError();
