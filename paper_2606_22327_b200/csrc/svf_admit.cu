@@ -129,13 +129,27 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
     const int E = R + Kc;
     int rem_l[AP_IPT];
     int maxrem = 0;
+    {   // two rounds of independent loads (the candidates' (s, o) are gathered through their sorted words)
+        uint32_t h[AP_IPT];
+        int kvv[AP_IPT];
 #pragma unroll
-    for (int i = 0; i < AP_IPT; ++i) {
-        const int e = tid + i * AP_THREADS;
-        rem_l[i] = 0;
-        if (e < R) { kv_e[e] = r_kv[e]; rem_l[i] = r_rem[e]; }
-        else if (e < E) { const uint32_t h = (uint32_t)wsorted[e - R]; kv_e[e] = w_s[h]; rem_l[i] = w_o[h]; }
-        maxrem = rem_l[i] > maxrem ? rem_l[i] : maxrem;
+        for (int i = 0; i < AP_IPT; ++i) {
+            const int e = tid + i * AP_THREADS;
+            h[i] = (e >= R && e < E) ? (uint32_t)wsorted[e - R] : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) {
+            const int e = tid + i * AP_THREADS;
+            const bool run = e < R, cand = e >= R && e < E;
+            kvv[i] = run ? r_kv[e] : (cand ? w_s[h[i]] : 0);
+            rem_l[i] = run ? r_rem[e] : (cand ? w_o[h[i]] : 0);
+        }
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) {
+            const int e = tid + i * AP_THREADS;
+            if (e < E) kv_e[e] = kvv[i];
+            maxrem = rem_l[i] > maxrem ? rem_l[i] : maxrem;
+        }
     }
     maxrem = __reduce_max_sync(FULL, maxrem);
     if (tid < 2) red_s[tid] = 0;
@@ -211,11 +225,45 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         return __syncthreads_or(bad) == 0;               // also fences wsum_s / wcnt_s for the next call
     };
     static_assert(WARPS == 32, "the second scan level holds one warp total per lane");
+    // the same probe in 32 bits when the numbers allow it (M < 2^26 and rem * count < 2^30: every config
+    // of the paper's shape): sums SATURATE at 2^26 > M (all terms are >= 0, so a saturated sum is a
+    // violated one and saturating addition stays associative), one shuffle per scan step instead of
+    // three, and the warp totals are combined by one hardware reduction
+    constexpr uint32_t SAT = 1u << 26;
+    const bool narrow = M < (int64_t)SAT && (int64_t)maxrem * E < ((int64_t)1 << 30);
+    __shared__ uint32_t wsum32_s[WARPS];
+    auto feasible32 = [&](int m) -> bool {
+        uint32_t s = 0; int c = 0;
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i) if (rk[i] < m) { s += (uint32_t)kv[i]; s = s < SAT ? s : SAT; ++c; }
+        uint32_t packed_c = (uint32_t)c;
+        uint32_t si = s; uint32_t ci = packed_c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t x = __shfl_up_sync(FULL, si, d), y = __shfl_up_sync(FULL, ci, d);
+            if (lane >= d) { si += x; si = si < SAT ? si : SAT; ci += y; }
+        }
+        if (lane == 31) { wsum32_s[wrp] = si; wcnt_s[wrp] = (int)ci; }
+        __syncthreads();
+        // exclusive prefix over the warps before mine: 32 warp totals <= 2^26 each sum below 2^31
+        const uint32_t wv = lane < wrp ? wsum32_s[lane] : 0u;
+        const int wcv = lane < wrp ? wcnt_s[lane] : 0;
+        uint32_t pre = __reduce_add_sync(FULL, wv); pre = pre < SAT ? pre : SAT;
+        int cnt = __reduce_add_sync(FULL, wcv);
+        pre += si - s; pre = pre < SAT ? pre : SAT;          // (si - s: this warp's lanes before mine, saturated alike)
+        cnt += (int)ci - c;
+        bool bad = false;
+        const uint32_t Mu = (uint32_t)M;
+#pragma unroll
+        for (int i = 0; i < AP_IPT; ++i)
+            if (rk[i] < m) { pre += (uint32_t)kv[i]; pre = pre < SAT ? pre : SAT; ++cnt; bad |= pre + (uint32_t)rem[i] * (uint32_t)cnt > Mu; }
+        return __syncthreads_or(bad) == 0;
+    };
 
     int lo = 0, hi = Kc + 1;                                 // feasible(lo) (or nobody fits at all), !feasible(hi)
     while (hi - lo > 1) {
         const int mid = (lo + hi) >> 1;
-        if (feasible(mid)) lo = mid; else hi = mid;
+        if (narrow ? feasible32(mid) : feasible(mid)) lo = mid; else hi = mid;
     }
     if (lo == Kc && (int64_t)Kc < n_wait) {
         // every candidate held here fits and more are waiting: the serial kernels take over; give

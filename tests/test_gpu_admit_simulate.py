@@ -388,6 +388,11 @@ def test_admit_prefix_bisection_and_its_handover(B, oracle):
     assert 8092 < k < 20_000
     st = _admit_state(6, 3000, 4097, 8_000_000)
     assert _admit_both(B, oracle, 0, 8_000_000, st) > 0                # n_run > 4096: serial path
+    # the probe's 32-bit form needs M < 2^26 AND rem * count < 2^30; very long remaining times take the 64-bit form
+    w_s, w_o, w_a, w_bit, r_kv, r_rem = _admit_state(8, 6000, 40, 1_000_000)
+    long_rem = (r_rem.astype(np.int64) * 4000).astype(np.int32)        # up to 12,000,000 steps left
+    for M in (60_000_000, 700_000_000, 2_000_000_000):
+        assert _admit_both(B, oracle, 2, M, (w_s, w_o, w_a, w_bit, r_kv, long_rem)) >= 0
     w_s, w_o, w_a, w_bit, r_kv, r_rem = _admit_state(7, 500, 50, 1_000_000)
     r_kv = r_kv.copy(); r_kv[0] = 999_990                              # running set alone already over M at its first completion
     assert _admit_both(B, oracle, 0, 1_000_000, (w_s, w_o, w_a, w_bit, r_kv, r_rem)) == 0
