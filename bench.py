@@ -493,14 +493,17 @@ def admit_sweep(B, torch, dev, peak):
             # (8 B); the sort reads the words once for its histograms and reads + writes them once per
             # executed pass (26-bit keys: four 8-bit passes over [32, 64)); the sorted words are copied
             # out (16 B); the admission reads the running set and the first candidates (12 B each)
-            algo = W * (12 + 8 + 8 + 16 * 4 + 16) + (R + min(W, 8192 - R)) * 12
+            fused = W + R <= 8192          # the library then takes the whole decision in ONE launch on one CTA
+            algo = (W * (12 + 8 + 4) + R * 8) if fused else W * (12 + 8 + 8 + 16 * 4 + 16) + (R + min(W, 8192 - R)) * 12
             res.append({"W": W, "R": R, "ms": ms, "admitted": k, "launches": B.last_launch_count(1),
                         "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": W / ms * 1e3,
                         "phase_ms": {"keys_and_validation": float(ph[0]), "sorts": float(ph[1]), "admission": float(ph[2]),
                                      "whole_call_under_events": float(ph[3])},
                         "roofline": {"bound": "hbm", "achieved": algo / ms / 1e6, "peak": peak, "unit": "GB/s",
                                      "frac": algo / ms / 1e6 / peak, "algorithmic_bytes": algo,
-                                     "note": "a chain of ~14 small launches: launch latency, not bandwidth, sets the time at these sizes"}})
+                                     "note": ("one launch, one CTA: validation, keys, both sorts and the bisection in shared memory (the phase "
+                                              "split does not apply: all under 'admission'); bound by one SM's issue rate and barriers") if fused else
+                                             "a chain of 13 small launches: launch latency, not bandwidth, sets the time at these sizes"}})
     return res
 
 

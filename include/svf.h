@@ -121,7 +121,10 @@ int svf_keys(int policy, int64_t n, const int32_t* s, const int32_t* o, const in
  *                     may be NULL
  *   status_out        one int32: SVF_OK / SVF_ERANGE / SVF_EUNSORTED / SVF_EOVERFLOW; on error
  *                     k = 0
- * `t` only dates the decision (the check is relative to now).  0 <= n_wait, n_run < 2^30. */
+ * `t` only dates the decision (the check is relative to now).  0 <= n_wait, n_run < 2^30.
+ * Cost: n_wait + n_run <= 8192 (a serving queue): ONE kernel launch on one CTA; larger queues: keys +
+ * device-wide radix sort + one CTA that bisects the prefix length over the first 8192 - n_run
+ * candidates (serial continuation only if all of those fit and more are waiting). */
 size_t svf_admit_workspace_bytes(int64_t n_wait, int64_t n_run);
 int svf_admit(int policy, int64_t M, int32_t t,
               int64_t n_wait, const int32_t* w_s, const int32_t* w_o, const int32_t* w_a,

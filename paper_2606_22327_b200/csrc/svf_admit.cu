@@ -10,6 +10,8 @@
 //   entries in registers and BISECTS the prefix length m: one check = the completion-time form of
 //   the forward-looking test on running + {candidates of rank < m} = a masked block scan of
 //   (kv, count) + max, about a microsecond; 14 checks instead of thousands of serial admissions.
+//   A queue and a running set that fit the CTA together (n_wait + n_run <= 8192) take NOTHING else: the
+//   same kernel validates, computes the keys and sorts the queue in shared memory first (one launch).
 //   Only if all K_c candidates fit and more are waiting (or n_run > 4096) the serial path runs:
 //   k_admit: one CTA builds (f_j, A_j) in finish order with a block scan (svf_state.cuh) and checks
 //   the running set; then k_admit_slots (M < 2^30) takes the set into REGISTER SLOTS and pops the
@@ -88,6 +90,16 @@ constexpr size_t AP_SMEM = (size_t)2 * AP_CAP * 8 + (size_t)AP_CAP * 4 + (size_t
 
 // fast[0] = 1: this kernel has answered (outputs written); 0: the serial kernels must run, and
 // rsorted_out holds the running set in their order (latest finish first, ties in input order).
+// FUSED (n_wait + n_run <= 8192, the size of a real serving queue): the WHOLE decision in this one launch --
+// validation, keys (a1), packing (a2), the radix sort of the queue in shared memory (a3), then the
+// bisection; nothing else is launched.  Otherwise the queue arrives sorted by the device-wide sort.
+struct AdmitFused {
+    int policy; int32_t O0, O1;
+    const int32_t* w_a; const uint8_t* w_bit;
+    uint64_t* sorted_words_out;              // or NULL
+};
+
+template <bool FUSED>
 __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64_t n_wait, const int32_t* __restrict__ w_s,
                                                                 const int32_t* __restrict__ w_o, int n_run,
                                                                 const int32_t* __restrict__ r_kv,
@@ -97,7 +109,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
                                                                 uint64_t* __restrict__ rsorted_out, int* __restrict__ fast,
                                                                 int64_t* __restrict__ n_admitted_out,
                                                                 int32_t* __restrict__ admitted_idx_out,
-                                                                int32_t* __restrict__ status_out)
+                                                                int32_t* __restrict__ status_out, AdmitFused fu)
 {
     constexpr int WARPS = AP_THREADS / 32;
     extern __shared__ __align__(16) char ap_smem[];
@@ -112,19 +124,73 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
     __shared__ int red_s[2];
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
 
+    const int R = n_run;
     int32_t status = SVF_OK;
-    if (fl->first_bad != ~0ull) status = (fl->first_bad & 1ull) ? SVF_EUNSORTED : SVF_ERANGE;
-    else if (fl->run_bad) status = SVF_ERANGE;
-    else if (fl->key_status != SVF_OK) status = fl->key_status;
+    if (!FUSED) {
+        if (fl->first_bad != ~0ull) status = (fl->first_bad & 1ull) ? SVF_EUNSORTED : SVF_ERANGE;
+        else if (fl->run_bad) status = SVF_ERANGE;
+        else if (fl->key_status != SVF_OK) status = fl->key_status;
+    } else {
+        // validation (first offending waiting index: range before order at the same index; then the
+        // running set; then the key width), keys and packed words, all on this CTA
+        __shared__ unsigned long long first_bad_s;
+        __shared__ uint32_t vflags_s[2];                    // [0] running set out of range, [1] OR of the keys' high words
+        if (tid == 0) { first_bad_s = ~0ull; vflags_s[0] = 0; vflags_s[1] = 0; }
+        if (tid < 2) red_s[tid] = 0;
+        __syncthreads();
+        unsigned long long bad = ~0ull;
+        uint32_t kor = 0, khi = 0, rb = 0;
+        const int nw = (int)n_wait;
+        for (int i = tid; i < nw; i += AP_THREADS) {
+            const int32_t si = w_s[i], oi = w_o[i], ai = fu.w_a[i];
+            unsigned long long b = ~0ull;
+            if (oi < 1 || si < 0 || ai < 0) b = (unsigned long long)i << 1;
+            else if (i > 0 && ai < fu.w_a[i - 1]) b = ((unsigned long long)i << 1) | 1ull;
+            bad = b < bad ? b : bad;
+            const uint32_t bt = fu.policy == SVF_SVF_1BIT ? (uint32_t)fu.w_bit[i] : 0u;
+            const uint64_t key = (oi >= 1 && si >= 0 && ai >= 0) ? priority_key(fu.policy, si, oi, ai, bt, fu.O0, fu.O1) : 0ull;
+            khi |= (uint32_t)(key >> 32);
+            kor |= (uint32_t)key;
+            buf0[i] = (key << 32) | (uint32_t)i;
+        }
+        for (int i = tid; i < R; i += AP_THREADS) if (r_rem[i] < 1 || r_kv[i] < 0) rb = 1;
+        if (bad != ~0ull) atomicMin(&first_bad_s, bad);
+        if (rb) atomicOr(&vflags_s[0], 1u);
+        khi = __reduce_or_sync(FULL, khi); kor = __reduce_or_sync(FULL, kor);
+        if (lane == 0) { if (khi) atomicOr(&vflags_s[1], khi); if (kor) atomicOr(reinterpret_cast<unsigned int*>(&red_s[1]), kor); }
+        __syncthreads();
+        if (first_bad_s != ~0ull) status = (first_bad_s & 1ull) ? SVF_EUNSORTED : SVF_ERANGE;
+        else if (vflags_s[0]) status = SVF_ERANGE;
+        else if (vflags_s[1]) status = SVF_EOVERFLOW;
+    }
     if (status != SVF_OK) {
-        if (tid == 0) { *n_admitted_out = 0; if (status_out) *status_out = status; *fast = 1; }
+        if (tid == 0) { *n_admitted_out = 0; if (status_out) *status_out = status; if (fast) *fast = 1; }
         return;
+    }
+    if (FUSED) {
+        // a3: the queue in priority order: stable radix passes over the significant key bytes; the order
+        // is kept as the input indices at kv_e[R + rank] (overwritten in place by kv below)
+        const int nw = (int)n_wait;
+        const uint32_t kall = (uint32_t)red_s[1];
+        const int npass = ((kall ? 32 - __clz(kall) : 0) + SORT_RADIX_BITS - 1) / SORT_RADIX_BITS;
+        const int ipt = (nw + AP_THREADS - 1) / AP_THREADS;
+        for (int p = 0; p < npass; ++p) {
+            seg_pass<AP_THREADS, AP_IPT>(buf0, buf1, nw, ipt, 32 + p * SORT_RADIX_BITS, whist, toff_s, warp_tot);
+            uint64_t* tmp = buf0; buf0 = buf1; buf1 = tmp;
+        }
+        __syncthreads();
+        for (int i = tid; i < nw; i += AP_THREADS) {
+            const uint64_t w = buf0[i];
+            kv_e[R + i] = (int32_t)(uint32_t)w;
+            if (fu.sorted_words_out) fu.sorted_words_out[i] = w;
+            if (admitted_idx_out) admitted_idx_out[i] = (int32_t)(uint32_t)w;      // the first k of them are the answer
+        }
+        __syncthreads();
     }
 
     // entries: e < R the running set as given (kv, rem); e >= R the candidate of priority rank e - R,
     // started now: it holds s now and has o steps left
-    const uint64_t* __restrict__ wsorted = wplan->result;
-    const int R = n_run;
+    const uint64_t* __restrict__ wsorted = FUSED ? nullptr : wplan->result;
     const int Kc = (int)(n_wait < (int64_t)(AP_CAP - R) ? n_wait : (int64_t)(AP_CAP - R));
     const int E = R + Kc;
     int rem_l[AP_IPT];
@@ -135,7 +201,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
 #pragma unroll
         for (int i = 0; i < AP_IPT; ++i) {
             const int e = tid + i * AP_THREADS;
-            h[i] = (e >= R && e < E) ? (uint32_t)wsorted[e - R] : 0u;
+            h[i] = (e >= R && e < E) ? (FUSED ? (uint32_t)kv_e[e] : (uint32_t)wsorted[e - R]) : 0u;
         }
 #pragma unroll
         for (int i = 0; i < AP_IPT; ++i) {
@@ -152,6 +218,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         }
     }
     maxrem = __reduce_max_sync(FULL, maxrem);
+    __syncthreads();                           // (FUSED: every thread has read its candidates' indices out of kv_e)
     if (tid < 2) red_s[tid] = 0;
     __syncthreads();
     if (lane == 0) atomicMax(&red_s[0], maxrem);
@@ -265,7 +332,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         const int mid = (lo + hi) >> 1;
         if (narrow ? feasible32(mid) : feasible(mid)) lo = mid; else hi = mid;
     }
-    if (lo == Kc && (int64_t)Kc < n_wait) {
+    if (!FUSED && lo == Kc && (int64_t)Kc < n_wait) {
         // every candidate held here fits and more are waiting: the serial kernels take over; give
         // them the running set in finish order (its entries, compacted from the order above)
         int c = 0;
@@ -290,9 +357,9 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         if (tid == 0) *fast = 0;
         return;
     }
-    if (admitted_idx_out)
+    if (!FUSED && admitted_idx_out)
         for (int k = tid; k < lo; k += AP_THREADS) admitted_idx_out[k] = (int32_t)(uint32_t)wsorted[k];
-    if (tid == 0) { *n_admitted_out = lo; if (status_out) *status_out = SVF_OK; *fast = 1; }
+    if (tid == 0) { *n_admitted_out = lo; if (status_out) *status_out = SVF_OK; if (fast) *fast = 1; }
 }
 
 __global__ void __launch_bounds__(ADMIT_THREADS) k_admit(int64_t M, int32_t t, int64_t n_wait,
@@ -555,6 +622,18 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
 
     g_admit_events_valid = false;
     admit_mark(0, st);
+    if (n_wait + n_run <= AP_CAP) {
+        // a queue and a running set that fit one CTA's shared memory: the whole decision in ONE launch
+        AdmitFused fu{policy, O0, O1, w_a, w_bit, sorted_words_out};
+        if (cudaFuncSetAttribute(k_admit_prefix<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
+        admit_mark(1, st);
+        admit_mark(2, st);
+        k_admit_prefix<true><<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, nullptr, nullptr, nullptr,
+                                                             nullptr, n_admitted_out, admitted_idx_out, status_out, fu);
+        ++g_launches_admit;
+        admit_mark(3, st);
+        return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
+    }
     k_admit_init<<<1, 1, 0, st>>>(w.flags);
     ++g_launches_admit;
     // a1 + a2
@@ -577,9 +656,9 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     const bool prefix = n_run <= AP_RUN_MAX;
     if (prefix) admit_mark(2, st);            // (else the running set's device-wide sort still belongs to phase 1)
     if (prefix) {
-        if (cudaFuncSetAttribute(k_admit_prefix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
-        k_admit_prefix<<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
-                                                       w.fast, n_admitted_out, admitted_idx_out, status_out);
+        if (cudaFuncSetAttribute(k_admit_prefix<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
+        k_admit_prefix<false><<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
+                                                              w.fast, n_admitted_out, admitted_idx_out, status_out, AdmitFused{});
         ++g_launches_admit;
     } else {
         rc = sort_u64(w.rsort, w.r0, w.r1, w.r0, n_run, 32, 64, st, &g_launches_admit);
