@@ -306,25 +306,56 @@ def run_ours(args):
     bounds = [S.strong_shard(batch.n_instances, c, n_chunks) for c in range(n_chunks)]
     subs = [batch.subset(range(lo, hi)) for lo, hi in bounds]
     streams = [torch.cuda.Stream(device=dev) for _ in range(n_chunks)]
-    pinned, c_outs, c_ws, host_out = [], [], [], []
+    # Per chunk ONE pinned host block and ONE device block for the five trace arrays, ONE device block
+    # and ONE pinned host block for every output of every policy: a chunk is one H2D copy, one call,
+    # one D2H copy (the C ABI takes plain pointers: the arrays are views into the blocks)
+    IN_FIELDS = (("offsets", torch.int64), ("arrival", torch.int32), ("prompt", torch.int32), ("output", torch.int32), ("bit", torch.uint8))
+
+    def carve(block, specs):
+        """views of `block` (uint8) for (name, dtype, numel) specs, each 256-byte aligned"""
+        views, off = {}, 0
+        for name, dt, numel in specs:
+            nbytes = numel * torch.empty(0, dtype=dt).element_size()
+            views[name] = block[off: off + nbytes].view(dt)
+            off += (nbytes + 255) // 256 * 256
+        return views
+
+    def block_bytes(specs):
+        return sum((numel * torch.empty(0, dtype=dt).element_size() + 255) // 256 * 256 for _, dt, numel in specs)
+
+    c_in_host, c_in_dev, c_trace, c_outs, c_out_dev, c_out_host, c_ws, host_out = [], [], [], [], [], [], [], []
+    h2d = d2h = 0
     for sub in subs:
-        pinned.append({k: torch.from_numpy(getattr(sub, k)).pin_memory() for k in ("offsets", "arrival", "prompt", "output", "bit")})
-        dsub = B.DeviceTrace.from_host(sub, device=dev)
-        c_outs.append([B.SimOut.alloc(dsub) for _ in POLICIES])
-        c_ws.append(torch.empty(B.svf_simulate_policies_workspace_bytes(dsub, len(POLICIES)), dtype=torch.uint8, device=dev))
-        host_out.append([{k: torch.empty_like(getattr(o, k), device="cpu").pin_memory() for k in B.RESULT_FIELDS}
-                         for o in c_outs[-1]])
-    h2d = sum(int(v.numel() * v.element_size()) for pc in pinned for v in pc.values())
-    d2h = sum(int(v.numel() * v.element_size()) for hc in host_out for ho in hc for v in ho.values())
+        in_specs = [(k, dt, int(getattr(sub, k).size)) for k, dt in IN_FIELDS]
+        hb = torch.empty(block_bytes(in_specs), dtype=torch.uint8).pin_memory()
+        db = torch.empty(block_bytes(in_specs), dtype=torch.uint8, device=dev)
+        hv, dv = carve(hb, in_specs), carve(db, in_specs)
+        for k, _ in IN_FIELDS:
+            hv[k].copy_(torch.from_numpy(getattr(sub, k)))
+        c_in_host.append(hb); c_in_dev.append(db)
+        c_trace.append(B.DeviceTrace(dv["offsets"], dv["arrival"], dv["prompt"], dv["output"], dv["bit"], sub.n_instances,
+                                     sub.n_requests, sub.max_n, int(sub.O0), int(sub.O1), int(sub.M)))
+        h2d += int(hb.numel())
+        out_specs = []
+        for i in range(len(POLICIES)):
+            for k in B.RESULT_FIELDS:
+                dt = B._PER_REQUEST.get(k) or B._PER_INSTANCE[k]
+                out_specs.append((f"{i}.{k}", dt, max(sub.n_requests if k in B._PER_REQUEST else sub.n_instances, 1)))
+        ob = torch.empty(block_bytes(out_specs), dtype=torch.uint8, device=dev)
+        oh = torch.empty(block_bytes(out_specs), dtype=torch.uint8).pin_memory()
+        ov, ohv = carve(ob, out_specs), carve(oh, out_specs)
+        c_out_dev.append(ob); c_out_host.append(oh)
+        c_outs.append([B.SimOut(**{k: ov[f"{i}.{k}"] for k in B.RESULT_FIELDS}) for i in range(len(POLICIES))])
+        host_out.append([{k: ohv[f"{i}.{k}"] for k in B.RESULT_FIELDS} for i in range(len(POLICIES))])
+        c_ws.append(torch.empty(B.svf_simulate_policies_workspace_bytes(c_trace[-1], len(POLICIES)), dtype=torch.uint8, device=dev))
+        d2h += int(oh.numel())
 
     def e2e_step():
         for c in range(n_chunks):
             with torch.cuda.stream(streams[c]):
-                d = B.DeviceTrace.from_host(subs[c], device=dev, pinned=pinned[c], non_blocking=True)
-                B.svf_simulate_policies(d, POLICIES, outs=c_outs[c], ws=c_ws[c])
-                for i in range(len(POLICIES)):
-                    for k in B.RESULT_FIELDS:
-                        host_out[c][i][k].copy_(getattr(c_outs[c][i], k), non_blocking=True)
+                c_in_dev[c].copy_(c_in_host[c], non_blocking=True)
+                B.svf_simulate_policies(c_trace[c], POLICIES, outs=c_outs[c], ws=c_ws[c])
+                c_out_host[c].copy_(c_out_dev[c], non_blocking=True)
         torch.cuda.synchronize()
         return int(host_out[0][0]["total_latency"][0])
 

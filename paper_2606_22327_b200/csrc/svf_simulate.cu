@@ -406,7 +406,9 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     int threads = 32;
     if (c.slots) {
         const int64_t r_est = mx < M / 512 ? mx : M / 512;
-        if (r_est > 32 * SLOT_K && w >= 2) threads = 128;
+        // (an estimate just above the warp's 512 slots -- configs[2]: 585, peaks of 530 -- is served better by
+        // the warp and a few ext slots unless warps are plentiful; far above it the CTA wins even at w = 2)
+        if ((r_est > 32 * SLOT_K && w >= 4) || (r_est > 48 * SLOT_K && w >= 2)) threads = 128;
         if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
     } else {
         while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
