@@ -157,8 +157,14 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
 }
 // QREG: shared memory holds the (s, o) records by rank and the bitmap mirror; the ext slots
 // (touched only when more than 32*K requests run at once) live in a global slot per CTA
+// (QW bitmap words per lane: 1,024 ranks each; QW = 1 for the bench shape, 2 for instances up to 2,048)
 constexpr int QREG_RANKS = 1024;
-constexpr size_t QREG_SMEM_BYTES = (size_t)QREG_RANKS * 8 + 32 * 4 + 32 * 8;   // (s, o) by rank, bitmap mirror, output buffer
+constexpr int QREG_MAX_WORDS = 2;
+__host__ __device__ constexpr size_t qreg_smem_bytes(int qw)      // (s, o) by rank, bitmap mirror, output buffer
+{
+    return (size_t)QREG_RANKS * qw * 8 + (size_t)32 * qw * 4 + 32 * 8;
+}
+constexpr size_t QREG_SMEM_BYTES = qreg_smem_bytes(1);
 __host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
 
 // one reduction round over the group: a summed (mod 2^32), b maxed, c minned; uniform afterwards
@@ -327,9 +333,11 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #ifndef SVF_WARP_MIN_CTAS
 #define SVF_WARP_MIN_CTAS 19
 #endif
-template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG>
-__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MIN_CTAS : 1) k_sim_slots(SlotArgs g)
+template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG, int QW = 1>
+__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? SVF_WARP_MIN_CTAS : 12) : 1) k_sim_slots(SlotArgs g)
 {
+    static_assert(QW >= 1 && QW <= QREG_MAX_WORDS && (QREG || QW == 1), "QW: bitmap words per lane of the register queue");
+    constexpr int QRANKS = QREG_RANKS * QW;
     static_assert(K == 16, "SVF_SLOT_GROUPS / SVF_PUT16 are written out for 16 register slots per thread");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
     using G = Group<THREADS>;
@@ -361,8 +369,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
     uint32_t* eB = reinterpret_cast<uint32_t*>(ebase + estride);
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
-    uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QREG_RANKS * 8);  // QREG only
-    int2* obuf = reinterpret_cast<int2*>(dyn_smem + (size_t)QREG_RANKS * 8 + 32 * 4);  // QREG only: (rank, start) of the last <= 32 admissions
+    uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QRANKS * 8);  // QREG only: [32 QW] words
+    int2* obuf = reinterpret_cast<int2*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4);  // QREG only: (rank, start) of the last <= 32 admissions
     const int Mi = (int)g.M;
     const int64_t n_items = g.I * g.n_policies;
     const uint32_t one = g.n_policies > 0 ? 1u : 0u;      // 1, but not to the compiler (SVF_ACC_GE)
@@ -384,7 +392,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
         const int64_t n64 = g.off[j + 1] - base;
         uint32_t flags = 0;
         if (n64 < 0 || n64 > g.max_instance || base < 0 || base + (n64 > 0 ? n64 : 0) > g.N ||
-            g.off[0] != 0 || g.off[g.I] != g.N || (QREG && n64 > QREG_RANKS) || *g.layout_bad)
+            g.off[0] != 0 || g.off[g.I] != g.N || (QREG && n64 > QRANKS) || *g.layout_bad)
             flags |= F_LAYOUT;
         const int n = (flags & F_LAYOUT) ? 0 : (int)n64;
         const int32_t* __restrict__ a = g.a + base;
@@ -407,7 +415,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
             // QREG: the (s, o) of every request by RANK in shared memory, once per instance (the presort
             // wrote a permutation of [0, n) whatever the data was), so that picking a head never waits
             // for global memory
-            if (QREG) qrec[io.rank[base + i] & (QREG_RANKS - 1)] = make_int2(si, oi);
+            if (QREG) qrec[io.rank[base + i] & (QRANKS - 1)] = make_int2(si, oi);
         }
         flags = G::or_u32(flags, scratch, parity);
         sum_o = G::sum_i64(sum_o, scratch, parity);
@@ -435,7 +443,25 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
             int32_t* __restrict__ out_finish = io.finish + base;
             uint32_t* out_lat = io.lat + base;
             const int nL0 = (n + 31) / 32, nL1 = (nL0 + 31) / 32;
-            uint32_t qword = 0;                       // QREG: ranks [32 lane, 32 lane + 32); the register is the truth
+            // QREG: bitmap word w of this lane covers the ranks [32 (32 w + lane), + 32); the registers are the truth
+            uint32_t qword[QW];
+#pragma unroll
+            for (int w = 0; w < QW; ++w) qword[w] = 0;
+            // lowest waiting rank (INT_MAX if none), the rest of its word above it, the word's first rank
+            auto queue_head = [&](uint32_t& rest, int& wbase_) -> int {
+#pragma unroll
+                for (int w = 0; w < QW; ++w) {
+                    const uint32_t nz = __ballot_sync(FULL, qword[w] != 0u);
+                    if (nz) {
+                        const int l0 = __ffs(nz) - 1;
+                        const uint32_t w0 = __shfl_sync(FULL, qword[w], l0);
+                        wbase_ = (w * 32 + l0) * 32;
+                        rest = w0 & (w0 - 1u);
+                        return wbase_ + (__ffs(w0) - 1);
+                    }
+                }
+                return INT_MAX;
+            };
             if (!QREG) {
                 for (int i = tid; i < nL0; i += THREADS) L0[i] = 0;
                 for (int i = tid; i < nL1; i += THREADS) L1[i] = 0;
@@ -521,7 +547,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
                     if (!m) break;
                     if (QREG) {
                         // the arrivals of a step set their bits in a shared-memory copy of the bitmap
-                        if (!arrived) { qbits[lane] = qword; __syncwarp(); }
+                        if (!arrived) {
+#pragma unroll
+                            for (int w = 0; w < QW; ++w) qbits[w * 32 + lane] = qword[w];
+                            __syncwarp();
+                        }
                         if (v) atomicOr(&qbits[rw >> 5], 1u << (rw & 31));
                     } else {
                         // nobody may still be reading the bitmap for the previous step
@@ -554,12 +584,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
                     if (QREG) {
                         // reload the bitmap word; the head is its lowest set bit (arrivals set bits)
                         __syncwarp();
-                        qword = qbits[lane];
-                        const uint32_t nz = __ballot_sync(FULL, qword != 0u);
-                        const int l0 = __ffs(nz) - 1;
-                        const uint32_t w0 = __shfl_sync(FULL, qword, l0);
-                        const int r0 = l0 * 32 + (__ffs(w0) - 1);
-                        hbase = l0 * 32; hrest = w0 & (w0 - 1u);
+#pragma unroll
+                        for (int w = 0; w < QW; ++w) qword[w] = qbits[w * 32 + lane];
+                        const int r0 = queue_head(hrest, hbase);      // (arrivals set bits: the queue is not empty)
                         if (r0 != head.r) {
                             const int2 v = qrec[r0];
                             head.r = r0; head.s = v.x; head.o = v.y;
@@ -666,8 +693,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
                             peak = p2 > peak ? p2 : peak;
                         }
                         if (QREG) {
-                            const uint32_t hb = (uint32_t)head.r - (uint32_t)(lane << 5);
-                            if (hb < 32u) qword &= ~(1u << hb);
+#pragma unroll
+                            for (int w = 0; w < QW; ++w) {
+                                const uint32_t hb = (uint32_t)head.r - (uint32_t)((w * 32 + lane) << 5);
+                                if (hb < 32u) qword[w] &= ~(1u << hb);
+                            }
                             obuf[started & 31] = make_int2(head.r, t);     // every lane, same value: one broadcast store
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
@@ -684,12 +714,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? SVF_WARP_MI
                                 r = hbase + (__ffs(hrest) - 1);
                                 hrest &= hrest - 1u;
                             } else {
-                                const uint32_t nz = __ballot_sync(FULL, qword != 0u);
-                                if (!nz) { head.r = INT_MAX; break; }
-                                const int l0 = __ffs(nz) - 1;
-                                const uint32_t w0 = __shfl_sync(FULL, qword, l0);
-                                hbase = l0 * 32; hrest = w0 & (w0 - 1u);
-                                r = hbase + (__ffs(w0) - 1);
+                                r = queue_head(hrest, hbase);
+                                if (r == INT_MAX) { head.r = INT_MAX; break; }
                             }
                             const int2 v = qrec[r];
                             head.r = r; head.s = v.x; head.o = v.y;

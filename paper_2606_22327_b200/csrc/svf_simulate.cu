@@ -367,7 +367,8 @@ struct SimWs {
 struct SimConfig {
     bool slots;             // register-resident kernel (M < 2^30); else the wide sorted-array kernel
     int ecap, qcap;         // slots kernel: ext slots per instance, bitmap capacity
-    bool qreg;              // slots kernel: waiting bitmap in one register per lane (<= 1024 ranks)
+    bool qreg;              // slots kernel: waiting bitmap in registers, qw words per lane (<= 1024 qw ranks)
+    int qw;
     bool ext_global;        // slots kernel, one warp per item: bitmaps in shared memory, ext slots in a global slot
     size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
     size_t gslot_bytes;     // bytes of the per-CTA slot in global memory (0: none)
@@ -394,7 +395,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.sort_hi = c.sb + 32 + c.ib;
     c.cap = (int)((mx + 31) / 32 * 32);
     c.slots = M < ((int64_t)1 << 30);
-    c.ecap = 0; c.qcap = c.cap; c.qreg = false; c.ext_global = false;
+    c.ecap = 0; c.qcap = c.cap; c.qreg = false; c.qw = 1; c.ext_global = false;
     // group width.  Register-slot kernels: one WARP per item (512 register slots) unless the running
     // set can outgrow them and there are warps to spare: R is at most mx and, at a few hundred
     // tokens per running request, about M / 512.  Measured: a CTA-wide group is slower than a warp
@@ -408,7 +409,9 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
         const int64_t r_est = mx < M / 512 ? mx : M / 512;
         // (an estimate just above the warp's 512 slots -- configs[2]: 585, peaks of 530 -- is served better by
         // the warp and a few ext slots unless warps are plentiful; far above it the CTA wins even at w = 2)
-        if ((r_est > 32 * SLOT_K && w >= 4) || (r_est > 48 * SLOT_K && w >= 2)) threads = 128;
+        // and the register-queue warp kernel (instances up to 2,048 requests) beats the CTA at any w
+        const bool regq = mx <= QREG_RANKS * QREG_MAX_WORDS;
+        if ((r_est > 32 * SLOT_K && w >= 4 && !regq) || (r_est > 48 * SLOT_K && w >= 2)) threads = 128;
         if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
     } else {
         while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
@@ -418,12 +421,13 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.gslot_bytes = 0; c.max_cta_per_sm = 2;
     if (c.slots) {
         auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
-        c.qreg = threads == 32 && mx <= QREG_RANKS;
+        c.qreg = threads == 32 && mx <= QREG_RANKS * QREG_MAX_WORDS;
         if (c.qreg) {
             // records + bitmap mirror in shared memory, ext slots in a global slot per CTA
+            c.qw = mx <= QREG_RANKS ? 1 : 2;
             c.qcap = 0;
             c.ecap = ext_of(32);
-            c.state_bytes = QREG_SMEM_BYTES;
+            c.state_bytes = qreg_smem_bytes(c.qw);
             c.smem = true;
             c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
             c.max_cta_per_sm = 32;
@@ -467,15 +471,15 @@ int sim_grid(const SimConfig& c, int64_t I)
     return (int)grid;
 }
 
-template <int THREADS, bool SMEM, bool QREG>
+template <int THREADS, bool SMEM, bool QREG, int QW = 1>
 int slots_grid(const SimConfig& c, int64_t I)
 {
     int per_sm = 0;
     if (SMEM) {
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true, QREG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
     }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG, QW>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
     int64_t grid = (int64_t)per_sm * sm_count();
     if (grid > I) grid = I;
@@ -486,7 +490,7 @@ int slots_grid(const SimConfig& c, int64_t I)
 int sim_grid_any(const SimConfig& c, int64_t I)
 {
     if (c.slots) {
-        if (c.qreg) return slots_grid<32, true, true>(c, I);
+        if (c.qreg) return c.qw == 2 ? slots_grid<32, true, true, 2>(c, I) : slots_grid<32, true, true, 1>(c, I);
         if (c.smem) {
             switch (c.threads) {
             case 32: return slots_grid<32, true, false>(c, I);
@@ -745,13 +749,14 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
         if (cudaMemsetAsync(w.counts, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return SVF_ECUDA;
         g_counts_dev = w.counts;
     }
-#define SVF_SLOTS_LAUNCH(T, S, Q)                                                         \
-    do {                                                                                  \
-        if (count) k_sim_slots<T, SLOT_K, S, true, Q><<<grid, T, c.dyn_smem, st>>>(q);    \
-        else       k_sim_slots<T, SLOT_K, S, false, Q><<<grid, T, c.dyn_smem, st>>>(q);   \
+#define SVF_SLOTS_LAUNCH(T, S, Q, ...)                                                              \
+    do {                                                                                            \
+        if (count) k_sim_slots<T, SLOT_K, S, true, Q, ##__VA_ARGS__><<<grid, T, c.dyn_smem, st>>>(q);   \
+        else       k_sim_slots<T, SLOT_K, S, false, Q, ##__VA_ARGS__><<<grid, T, c.dyn_smem, st>>>(q);  \
     } while (0)
     if (c.qreg) {
-        SVF_SLOTS_LAUNCH(32, true, true);
+        if (c.qw == 2) SVF_SLOTS_LAUNCH(32, true, true, 2);
+        else           SVF_SLOTS_LAUNCH(32, true, true, 1);
     } else if (c.smem) {
         switch (c.threads) {
         case 32: SVF_SLOTS_LAUNCH(32, true, false); break;
