@@ -250,6 +250,16 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     if ((g4) >= 2) { OP(7)  OP(6)  OP(5)  OP(4)  }                                            \
     if ((g4) >= 1) { OP(3)  OP(2)  OP(1)  OP(0)  }
 
+// the same for 32 register slots per thread (K = 32: 1,024 slots on one warp, for running sets that
+// outgrow 512 where a CTA-wide group would replicate the scalar part in every warp)
+#define SVF_SLOT_GROUPS32(g4, OP)                                                             \
+    if ((g4) >= 8) { OP(31) OP(30) OP(29) OP(28) }                                            \
+    if ((g4) >= 7) { OP(27) OP(26) OP(25) OP(24) }                                            \
+    if ((g4) >= 6) { OP(23) OP(22) OP(21) OP(20) }                                            \
+    if ((g4) >= 5) { OP(19) OP(18) OP(17) OP(16) }                                            \
+    SVF_SLOT_GROUPS(g4, OP)
+#define SVF_SLOTS(g4, OP) if constexpr (K == 32) { SVF_SLOT_GROUPS32(g4, OP) } else { SVF_SLOT_GROUPS(g4, OP) }
+
 // write into register slot ik (uniform) of the owning thread: a tree of uniform branches
 #define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
 #define SVF_PUT4(ik, OP, k0)  if ((ik) & 2) { SVF_PUT2(ik, OP, k0 + 2) } else { SVF_PUT2(ik, OP, k0) }
@@ -264,6 +274,8 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #else
 #define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
 #endif
+#define SVF_PUT32(ik, OP)     if ((ik) & 16) { if ((ik) & 8) { SVF_PUT8(ik, OP, 24) } else { SVF_PUT8(ik, OP, 16) } } else { SVF_PUT16(ik, OP) }
+#define SVF_PUTK(ik, OP)      if constexpr (K == 32) { SVF_PUT32(ik, OP) } else { SVF_PUT16(ik, OP) }
 
 // The per-slot operations of the passes.  They are macros over the LOCAL names of the calling
 // kernel (k_sim_slots here, k_admit_slots in svf_admit.cu): slots f[], B[], c[]; the head's t1 =
@@ -338,7 +350,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 {
     static_assert(QW >= 1 && QW <= QREG_MAX_WORDS && (QREG || QW == 1), "QW: bitmap words per lane of the register queue");
     constexpr int QRANKS = QREG_RANKS * QW;
-    static_assert(K == 16, "SVF_SLOT_GROUPS / SVF_PUT16 are written out for 16 register slots per thread");
+    static_assert(K == 16 || (K == 32 && THREADS == 32 && !QREG), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
     using G = Group<THREADS>;
     constexpr int WARPS = THREADS / 32;
@@ -611,12 +623,18 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
                         const int g4 = (kmax + 3) >> 2;
                         const bool use_ext = hw > REGCAP;
-                        SVF_SLOT_GROUPS(g4, SVF_EVAL)
+                        SVF_SLOTS(g4, SVF_EVAL)
                         // lowest free register slot of this thread as a one-hot bit (bit k of dm =
                         // slot k is dead); the group takes the lowest (slot, thread) pair
                         // (a sentinel bit marks the first slot past the groups in use; slot 16 = none)
-                        const uint32_t dmx = dm | (1u << (4 * g4));
-                        int fkey = (int)(((dmx & (0u - dmx)) << TSHIFT) | (uint32_t)tid);
+                        int fkey;
+                        if constexpr (K == 32) {      // 32 slots: the key carries the slot NUMBER (32 = none)
+                            const uint32_t dmx = dm | (g4 < 8 ? (1u << (4 * g4)) : 0u);
+                            fkey = ((dmx ? __ffs(dmx) - 1 : K) << TSHIFT) | tid;
+                        } else {
+                            const uint32_t dmx = dm | (1u << (4 * g4));
+                            fkey = (int)(((dmx & (0u - dmx)) << TSHIFT) | (uint32_t)tid);
+                        }
                         int eidx = INT_MAX;
                         if (use_ext) {
                             for (int q = REGCAP + tid; q < hw; q += THREADS) {
@@ -642,7 +660,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                             // long the head stays blocked at least --------------------------------
                             int wmax = 0, minge = INT_MAX;
                             if (COUNT) ++cntBk;
-                            if (Ah > Mi) { SVF_SLOT_GROUPS(g4, SVF_BLOCK) } else { SVF_SLOT_GROUPS(g4, SVF_BLOCK2) }
+                            if (Ah > Mi) { SVF_SLOTS(g4, SVF_BLOCK) } else { SVF_SLOTS(g4, SVF_BLOCK2) }
                             if (use_ext) {
                                 for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                     const int e = q - REGCAP;
@@ -669,11 +687,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         // ---- admitted: the update is already in place; write the head into a slot --
                         const uint32_t Bh = (uint32_t)Ah + fhu;
                         int idx;
-                        if (fkey < (1 << (K + TSHIFT))) {
-                            const int ik = 31 - __clz(fkey >> TSHIFT);           // uniform
+                        if (K == 32 ? fkey < (K << TSHIFT) : fkey < (1 << (K + TSHIFT))) {
+                            const int ik = K == 32 ? (fkey >> TSHIFT) : 31 - __clz(fkey >> TSHIFT);           // uniform
                             const bool mine = (fkey & (THREADS - 1)) == tid;
                             idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
-                            SVF_PUT16(ik, SVF_PUT)
+                            SVF_PUTK(ik, SVF_PUT)
                         } else {
                             // every register slot is live: the lowest dead ext slot, else a new one
                             if (use_ext) {

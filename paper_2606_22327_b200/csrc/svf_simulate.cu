@@ -370,6 +370,7 @@ struct SimConfig {
     bool qreg;              // slots kernel: waiting bitmap in registers, qw words per lane (<= 1024 qw ranks)
     int qw;
     bool ext_global;        // slots kernel, one warp per item: bitmaps in shared memory, ext slots in a global slot
+    int k;                  // slots kernel: register slots per thread (16; 32: one warp with 1,024 slots)
     size_t state_bytes;     // per-CTA state (shared memory, or a global slot when smem is false)
     size_t gslot_bytes;     // bytes of the per-CTA slot in global memory (0: none)
     int max_cta_per_sm;     // bound on resident CTAs per SM (sizes the global slots)
@@ -395,7 +396,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.sort_hi = c.sb + 32 + c.ib;
     c.cap = (int)((mx + 31) / 32 * 32);
     c.slots = M < ((int64_t)1 << 30);
-    c.ecap = 0; c.qcap = c.cap; c.qreg = false; c.qw = 1; c.ext_global = false;
+    c.ecap = 0; c.qcap = c.cap; c.qreg = false; c.qw = 1; c.ext_global = false; c.k = SLOT_K;
     // group width.  Register-slot kernels: one WARP per item (512 register slots) unless the running
     // set can outgrow them and there are warps to spare: R is at most mx and, at a few hundred
     // tokens per running request, about M / 512.  Measured: a CTA-wide group is slower than a warp
@@ -413,6 +414,10 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
         const bool regq = mx <= QREG_RANKS * QREG_MAX_WORDS;
         if ((r_est > 32 * SLOT_K && w >= 4 && !regq) || (r_est > 48 * SLOT_K && w >= 2)) threads = 128;
         if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
+        // ... unless ONE warp with 32 slots per thread holds the set (estimates up to 1,600: the estimate
+        // counts 512 tokens per running request, real sets are smaller): no barrier, no scalar part
+        // replicated in four warps (configs[4] at M = 800k: 10.4 ms with CTAs)
+        if (threads == 128 && r_est <= 100 * SLOT_K) { threads = 32; c.k = 32; }
     } else {
         while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
         if (threads == 64) threads = 128;
@@ -420,8 +425,8 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     }
     c.gslot_bytes = 0; c.max_cta_per_sm = 2;
     if (c.slots) {
-        auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * SLOT_K; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
-        c.qreg = threads == 32 && mx <= QREG_RANKS * QREG_MAX_WORDS;
+        auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * c.k; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
+        c.qreg = threads == 32 && c.k == SLOT_K && mx <= QREG_RANKS * QREG_MAX_WORDS;
         if (c.qreg) {
             // records + bitmap mirror in shared memory, ext slots in a global slot per CTA
             c.qw = mx <= QREG_RANKS ? 1 : 2;
@@ -442,7 +447,7 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
             c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
             c.max_cta_per_sm = 32;
         } else {
-            if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) threads = 128;
+            if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT) { threads = 128; c.k = SLOT_K; }
             c.ecap = ext_of(threads);
             c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
             c.smem = c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
@@ -471,15 +476,15 @@ int sim_grid(const SimConfig& c, int64_t I)
     return (int)grid;
 }
 
-template <int THREADS, bool SMEM, bool QREG, int QW = 1>
+template <int THREADS, bool SMEM, bool QREG, int QW = 1, int KS = SLOT_K>
 int slots_grid(const SimConfig& c, int64_t I)
 {
     int per_sm = 0;
     if (SMEM) {
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
-        cudaFuncSetAttribute(k_sim_slots<THREADS, SLOT_K, SMEM, true, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, false, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, true, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
     }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, SLOT_K, SMEM, false, QREG, QW>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, KS, SMEM, false, QREG, QW>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
     int64_t grid = (int64_t)per_sm * sm_count();
     if (grid > I) grid = I;
@@ -491,6 +496,7 @@ int sim_grid_any(const SimConfig& c, int64_t I)
 {
     if (c.slots) {
         if (c.qreg) return c.qw == 2 ? slots_grid<32, true, true, 2>(c, I) : slots_grid<32, true, true, 1>(c, I);
+        if (c.k == 32) return slots_grid<32, true, false, 1, 32>(c, I);
         if (c.smem) {
             switch (c.threads) {
             case 32: return slots_grid<32, true, false>(c, I);
@@ -757,6 +763,9 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
     if (c.qreg) {
         if (c.qw == 2) SVF_SLOTS_LAUNCH(32, true, true, 2);
         else           SVF_SLOTS_LAUNCH(32, true, true, 1);
+    } else if (c.k == 32) {
+        if (count) k_sim_slots<32, 32, true, true, false><<<grid, 32, c.dyn_smem, st>>>(q);
+        else       k_sim_slots<32, 32, true, false, false><<<grid, 32, c.dyn_smem, st>>>(q);
     } else if (c.smem) {
         switch (c.threads) {
         case 32: SVF_SLOTS_LAUNCH(32, true, false); break;

@@ -221,12 +221,14 @@ def test_random_small_instances_all_policies(B, oracle):
 
 
 def test_group_widths_and_state_placement(B, oracle):
-    """Shapes that select the warp kernel and the CTA kernels (the 256-thread one: see the crowd test)."""
-    shapes = [(200, 1300, 4.0),        # one warp each, shared-memory bitmap (more than 1024 requests)
+    """Shapes that select each form of the one-warp kernel (M = 60,000: few requests run at once); the
+    CTA-wide kernels and the 32-slot warp kernel are in the crowd test, configs[3] and configs[4]."""
+    shapes = [(200, 1300, 4.0),        # one warp each, two bitmap words per lane (more than 1024 requests)
+              (100, 2500, 8.0),        # one warp each, shared-memory bitmap (more than 2048 requests)
               (4096 // 8, 40, 2.0),     # many small instances -> one warp each
-              (100, 600, 4.0),         # 128 threads
-              (1, 2000, 4.0),          # 256 threads
-              (2, 9000, 8.0)]          # 1024 threads, shared state
+              (100, 600, 4.0),         # register queue, one bitmap word per lane
+              (1, 2000, 4.0),          # a single instance: register queue, two words per lane
+              (2, 9000, 8.0)]          # shared-memory bitmap, ext slots in the global slot
     for I, n, lam in shapes:
         tr = T.config3(n_instances=I, n=n, lam=lam, M=60_000)
         for policy in (0, 3):
@@ -507,7 +509,8 @@ def test_more_running_requests_than_register_slots(B, oracle):
             o = T.uniform_int(sd, 3, n, 150, 400)
             parts.append(T._one("", a, s, o, (o > 250).astype(np.uint8), 0, 200, 300))
         return parts
-    for I, n, M in ((40, 1000, 330_000), (600, 900, 200_000), (3, 5000, 1_500_000), (1, 9000, 2_500_000)):
+    # (40 x 1500 at M = 800k: the one-warp kernel with 32 slots per thread, 1,024 register slots, the rest in ext slots)
+    for I, n, M in ((40, 1000, 330_000), (600, 900, 200_000), (40, 1500, 800_000), (3, 5000, 1_500_000), (1, 9000, 2_500_000)):
         tr = T.concat(crowd(I, n, n), f"crowd{I}x{n}", M, 200, 300)
         for policy in (0, 1, 3):
             ref, got = check(B, oracle, tr, policy, ctx=f"{tr.name} policy {policy}")
