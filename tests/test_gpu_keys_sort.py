@@ -59,6 +59,22 @@ def test_keys_unaligned_views_take_the_scalar_path(B, oracle):
         assert np.array_equal(_u64(words), want)
 
 
+def test_keys_16_byte_aligned_views_take_the_128_bit_path(B, oracle):
+    """Arrays aligned to 16 but not to 32 bytes (and the words too): 128-bit accesses instead of the
+    256-bit ones a fresh allocation gets; ragged sizes for both tails."""
+    import torch
+    for n in (10_000, 10_003, 7):
+        s, o, a, bit = _rand_requests(6, n + 4)
+        ds, do, da, db = _dev(s)[4:n + 4], _dev(o)[4:n + 4], _dev(a)[4:n + 4], _dev(bit)[4:n + 4]
+        assert ds.data_ptr() % 32 == 16 and db.data_ptr() % 8 == 4
+        buf = torch.empty(n + 2, dtype=torch.int64, device="cuda")
+        for policy in range(4):
+            rc, want = oracle.keys(policy, s[4:n + 4], o[4:n + 4], a[4:n + 4], bit[4:n + 4], 5, 70)
+            words, status = B.svf_keys(policy, ds, do, da, db, 5, 70, words_out=buf[2:n + 2])
+            assert rc == 0 and int(status.item()) == 0
+            assert np.array_equal(_u64(words), want)
+
+
 def test_keys_overflow_is_reported(B, oracle):
     s = np.array([1, 65536, 7, 9, 2], np.int32)
     o = np.array([1, 65536, 7, 9, 3], np.int32)
