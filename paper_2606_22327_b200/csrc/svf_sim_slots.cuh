@@ -162,7 +162,7 @@ constexpr int QREG_RANKS = 1024;
 constexpr int QREG_MAX_WORDS = 2;
 __host__ __device__ constexpr size_t qreg_smem_bytes(int qw)      // (s, o) by rank, bitmap mirror, output buffer
 {
-    return (size_t)QREG_RANKS * qw * 8 + (size_t)32 * qw * 4 + 32 * 8;
+    return (size_t)QREG_RANKS * qw * 8 + (size_t)32 * qw * 4 + 32 * 8 + 32 * 8 + 32 * 4;   // + per-lane latency sums and makespans
 }
 constexpr size_t QREG_SMEM_BYTES = qreg_smem_bytes(1);
 __host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
@@ -383,6 +383,21 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
     uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QRANKS * 8);  // QREG only: [32 QW] words
     int2* obuf = reinterpret_cast<int2*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4);  // QREG only: (rank, start) of the last <= 32 admissions
+    // QREG only: the per-lane latency sums and makespans live in shared memory (touched once per 32
+    // admissions), not in three registers across the hot loop
+    long long* tel_s = reinterpret_cast<long long*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4 + 32 * 8);
+    int* mk_s = reinterpret_cast<int*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4 + 32 * 8 + 32 * 8);
+    // QREG: the shared-memory window address of dyn_smem, held in ONE register (opaque to the compiler,
+    // which otherwise re-derives it from SR_CgaCtaId inside the hot loop)
+    uint32_t sm32 = 0;
+    if constexpr (QREG) {
+        sm32 = (uint32_t)__cvta_generic_to_shared(dyn_smem);
+        asm volatile("" : "+r"(sm32));
+    }
+    auto lds_rec = [&](int r) -> int2 {
+        int2 v; asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(sm32 + (uint32_t)r * 8u));
+        return v;
+    };
     const int Mi = (int)g.M;
     const int64_t n_items = g.I * g.n_policies;
     const uint32_t one = g.n_policies > 0 ? 1u : 0u;      // 1, but not to the compiler (SVF_ACC_GE)
@@ -503,6 +518,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 }
             };
             load_window();
+            if (QREG) { tel_s[lane] = 0; mk_s[lane] = 0; }
             auto win_rec = [&](int l, int r) {
                 Rec x; x.r = r; x.s = __shfl_sync(FULL, sw, l); x.o = __shfl_sync(FULL, ow, l);
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
@@ -525,8 +541,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         if (io_.start) io_.start[b_ + id] = e.y;
                         if (io_.finish) io_.finish[b_ + id] = fin;
                         if (io_.p99) io_.lat[b_ + id] = (uint32_t)lat;
-                        tel += lat;
-                        mk = fin > mk ? fin : mk;
+                        tel_s[lane] += lat;
+                        if (fin > mk_s[lane]) mk_s[lane] = fin;
                     }
                 } else if (wrp == 0 && lane < count) {
                     const int id = b_id, lat = b_lat;
@@ -561,10 +577,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         // the arrivals of a step set their bits in a shared-memory copy of the bitmap
                         if (!arrived) {
 #pragma unroll
-                            for (int w = 0; w < QW; ++w) qbits[w * 32 + lane] = qword[w];
+                            for (int w = 0; w < QW; ++w)
+                                asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(w * 32 + lane) * 4u), "r"(qword[w]) : "memory");
                             __syncwarp();
                         }
-                        if (v) atomicOr(&qbits[rw >> 5], 1u << (rw & 31));
+                        if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(rw >> 5) * 4u), "r"(1u << (rw & 31)) : "memory");
                     } else {
                         // nobody may still be reading the bitmap for the previous step
                         if (!arrived) G::sync();
@@ -597,10 +614,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         // reload the bitmap word; the head is its lowest set bit (arrivals set bits)
                         __syncwarp();
 #pragma unroll
-                        for (int w = 0; w < QW; ++w) qword[w] = qbits[w * 32 + lane];
+                        for (int w = 0; w < QW; ++w)
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(qword[w]) : "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(w * 32 + lane) * 4u) : "memory");
                         const int r0 = queue_head(hrest, hbase);      // (arrivals set bits: the queue is not empty)
                         if (r0 != head.r) {
-                            const int2 v = qrec[r0];
+                            const int2 v = lds_rec(r0);
                             head.r = r0; head.s = v.x; head.o = v.y;
                             t_lb = t;                     // a new head: evaluate it now
                         }
@@ -716,7 +734,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                 const uint32_t hb = (uint32_t)head.r - (uint32_t)((w * 32 + lane) << 5);
                                 if (hb < 32u) qword[w] &= ~(1u << hb);
                             }
-                            obuf[started & 31] = make_int2(head.r, t);     // every lane, same value: one broadcast store
+                            // every lane, same value: one broadcast store
+                            asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)(QRANKS * 8 + 32 * QW * 4) + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
                             if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
@@ -735,7 +754,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                 r = queue_head(hrest, hbase);
                                 if (r == INT_MAX) { head.r = INT_MAX; break; }
                             }
-                            const int2 v = qrec[r];
+                            const int2 v = lds_rec(r);
                             head.r = r; head.s = v.x; head.o = v.y;
                         } else {
                             // promote the second; fetch the record behind it one admission ahead
@@ -767,6 +786,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 t = tn;
             }
             flush(started & 31);
+            if (QREG) { tel = tel_s[lane]; mk = mk_s[lane]; }
             decisions += (uint32_t)started;
             if (want_p99) {                       // nearest rank ceil(0.99 n), 1-based (R13)
                 G::sync();
