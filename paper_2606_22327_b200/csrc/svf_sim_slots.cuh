@@ -43,11 +43,14 @@
 // exactly as the step-by-step definition counts them (one blocked-head evaluation each).
 //
 // WAITING QUEUE: bitmap over ranks (keys are time-invariant, so the presort fixes the order).
-//  * QREG (one warp per instance, at most 1024 requests): one 32-bit word per lane in a register,
-//    mirrored in shared memory where arrivals set their bits with one atomicOr each; the (s, o) of
-//    every waiting request sits in shared memory by rank (8 KB), written on arrival, so picking
-//    the next head never waits for global memory; id and arrival are only looked up when the
-//    outputs are written.
+//  * QREG (one warp per instance, at most 8,192 requests): QW 32-bit words per lane in registers
+//    (QW = 1, 2 or 8: 1,024 ranks per word index), mirrored in shared memory where arrivals set their
+//    bits with one atomic OR each; the (s, o) of every request sits in shared memory by rank, staged
+//    once per instance, so picking the next head never waits for global memory; id and arrival are
+//    only looked up when the outputs are written.  Up to 2,048 requests the records are 8 bytes; above
+//    (REC4) they are PACKED into one word, s in the low bits, the split taken from the widths of the
+//    instance's own largest s and o (32 KB for 8,192 ranks: six warps per SM; an instance whose widths
+//    do not fit 32 bits together reads the records from global memory instead: correct, slower).
 //  * otherwise the two-level shared-memory bitmap of svf_state.cuh and (s, o, id, a) records in
 //    priority order in global memory.
 // The head of the queue is cached in registers (non-QREG: also the second, whose record is
@@ -157,12 +160,14 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
 }
 // QREG: shared memory holds the (s, o) records by rank and the bitmap mirror; the ext slots
 // (touched only when more than 32*K requests run at once) live in a global slot per CTA
-// (QW bitmap words per lane: 1,024 ranks each; QW = 1 for the bench shape, 2 for instances up to 2,048)
+// (QW bitmap words per lane: 1,024 ranks each; QW = 1 for the bench shape, 2 for instances up to 2,048,
+// 8 for instances up to 8,192, whose (s, o) records are PACKED into one 32-bit word each (REC4): 32 KB
+// instead of 64 KB per warp, six warps per SM instead of three)
 constexpr int QREG_RANKS = 1024;
-constexpr int QREG_MAX_WORDS = 2;
-__host__ __device__ constexpr size_t qreg_smem_bytes(int qw)      // (s, o) by rank, bitmap mirror, output buffer
+constexpr int QREG_MAX_WORDS = 8;
+__host__ __device__ constexpr size_t qreg_smem_bytes(int qw, bool rec4 = false)      // (s, o) by rank, bitmap mirror, output buffer
 {
-    return (size_t)QREG_RANKS * qw * 8 + (size_t)32 * qw * 4 + 32 * 8 + 32 * 8 + 32 * 4;   // + per-lane latency sums and makespans
+    return (size_t)QREG_RANKS * qw * (rec4 ? 4 : 8) + (size_t)32 * qw * 4 + 32 * 8 + 32 * 8 + 32 * 4;   // + per-lane latency sums and makespans
 }
 constexpr size_t QREG_SMEM_BYTES = qreg_smem_bytes(1);
 __host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
@@ -345,12 +350,15 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #ifndef SVF_WARP_MIN_CTAS
 #define SVF_WARP_MIN_CTAS 19
 #endif
-template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG, int QW = 1>
-__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? SVF_WARP_MIN_CTAS : 12) : 1) k_sim_slots(SlotArgs g)
+template <int THREADS, int K, bool SMEM, bool COUNT, bool QREG, int QW = 1, bool REC4 = false>
+__global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? SVF_WARP_MIN_CTAS : (QW == 2 ? 12 : 6)) : 1) k_sim_slots(SlotArgs g)
 {
     static_assert(QW >= 1 && QW <= QREG_MAX_WORDS && (QREG || QW == 1), "QW: bitmap words per lane of the register queue");
+    static_assert(!REC4 || QREG, "REC4: packed records of the register queue");
     constexpr int QRANKS = QREG_RANKS * QW;
-    static_assert(K == 16 || (K == 32 && THREADS == 32 && !QREG), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
+    constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
+    constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
+    static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
     using G = Group<THREADS>;
     constexpr int WARPS = THREADS / 32;
@@ -380,13 +388,13 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     int32_t* ef = reinterpret_cast<int32_t*>(ebase);
     uint32_t* eB = reinterpret_cast<uint32_t*>(ebase + estride);
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
-    int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only
-    uint32_t* qbits = reinterpret_cast<uint32_t*>(dyn_smem + (size_t)QRANKS * 8);  // QREG only: [32 QW] words
-    int2* obuf = reinterpret_cast<int2*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4);  // QREG only: (rank, start) of the last <= 32 admissions
+    int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only (REC4: one packed word per rank)
+    uint32_t* qrec4 = reinterpret_cast<uint32_t*>(dyn_smem);
+    int2* obuf = reinterpret_cast<int2*>(dyn_smem + OFF_OBUF);  // QREG only: (rank, start) of the last <= 32 admissions
     // QREG only: the per-lane latency sums and makespans live in shared memory (touched once per 32
     // admissions), not in three registers across the hot loop
-    long long* tel_s = reinterpret_cast<long long*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4 + 32 * 8);
-    int* mk_s = reinterpret_cast<int*>(dyn_smem + (size_t)QRANKS * 8 + 32 * QW * 4 + 32 * 8 + 32 * 8);
+    long long* tel_s = reinterpret_cast<long long*>(dyn_smem + OFF_TEL);
+    int* mk_s = reinterpret_cast<int*>(dyn_smem + OFF_MK);
     // QREG: the shared-memory window address of dyn_smem, held in ONE register (opaque to the compiler,
     // which otherwise re-derives it from SR_CgaCtaId inside the hot loop)
     uint32_t sm32 = 0;
@@ -394,10 +402,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
         sm32 = (uint32_t)__cvta_generic_to_shared(dyn_smem);
         asm volatile("" : "+r"(sm32));
     }
-    auto lds_rec = [&](int r) -> int2 {
-        int2 v; asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(sm32 + (uint32_t)r * 8u));
-        return v;
-    };
     const int Mi = (int)g.M;
     const int64_t n_items = g.I * g.n_policies;
     const uint32_t one = g.n_policies > 0 ? 1u : 0u;      // 1, but not to the compiler (SVF_ACC_GE)
@@ -428,7 +432,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 
         // ---- validation (data errors -> status[j], never UB) --------------------------------
         int64_t sum_o = 0;
-        int max_a = 0;
+        int max_a = 0, max_s = 0, max_o = 0;
         for (int i = tid; i < n; i += THREADS) {
             const int32_t ai = a[i], si = s[i], oi = o[i];
             const int32_t ki = g.okey ? g.okey[base + i] : oi;      // length the key sees
@@ -439,10 +443,12 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
             max_a = ai > max_a ? ai : max_a;
+            if (REC4) { max_s = si > max_s ? si : max_s; max_o = oi > max_o ? oi : max_o; }
             // QREG: the (s, o) of every request by RANK in shared memory, once per instance (the presort
             // wrote a permutation of [0, n) whatever the data was), so that picking a head never waits
             // for global memory
-            if (QREG) qrec[io.rank[base + i] & (QRANKS - 1)] = make_int2(si, oi);
+            // (REC4: packed below, once the widths are known)
+            if (QREG && !REC4) qrec[io.rank[base + i] & (QRANKS - 1)] = make_int2(si, oi);
         }
         flags = G::or_u32(flags, scratch, parity);
         sum_o = G::sum_i64(sum_o, scratch, parity);
@@ -463,6 +469,36 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 if (want_finish) io.finish[base + i] = -1;
             }
         } else {
+            // REC4: (s, o) of a waiting request packed into ONE word, s in the low `pshift` bits -- the
+            // widths are this instance's own (bits of its largest s and o); an instance whose widths
+            // do not fit 32 bits together (pshift < 0) leaves the records in global memory instead
+            int pshift = 0; uint32_t pmask = 0;
+            if constexpr (REC4) {
+                max_s = __reduce_max_sync(FULL, max_s); max_o = __reduce_max_sync(FULL, max_o);
+                const int bs = 32 - __clz(max_s), bo = 32 - __clz(max_o);
+                pshift = bs + bo <= 32 ? bs : -1;
+                pmask = pshift >= 0 ? (uint32_t)((1ull << pshift) - 1ull) : 0u;
+                if (pshift >= 0)
+                    for (int i = tid; i < n; i += THREADS)
+                        qrec4[io.rank[base + i] & (QRANKS - 1)] = (uint32_t)s[i] | ((uint32_t)o[i] << pshift);     // (pshift <= 31: s < 2^31)
+            }
+            auto lds_rec = [&](int r) -> int2 {
+                int2 v;
+                if constexpr (REC4) {
+                    if (pshift >= 0) {
+                        uint32_t x; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(x) : "r"(sm32 + (uint32_t)r * 4u));
+                        v.x = (int)(x & pmask); v.y = (int)(x >> pshift);
+                    } else {
+                        int pi_ = pi; long long b_ = base;
+                        asm volatile("" : "+r"(pi_), "+l"(b_));
+                        const int id = (int)g.io[pi_].order[b_ + r];
+                        v.x = g.s[b_ + id]; v.y = g.o[b_ + id];
+                    }
+                } else {
+                    asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(sm32 + (uint32_t)r * 8u));
+                }
+                return v;
+            };
             const uint32_t* __restrict__ rnk = io.rank + base;
             const uint32_t* __restrict__ ord = io.order + base;
             const int4* __restrict__ req = io.req + base;
@@ -537,7 +573,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         const PolicyIO& io_ = g.io[pi_];
                         const int2 e = obuf[lane];
                         const int id = (int)io_.order[b_ + e.x];
-                        const int fin = e.y + qrec[e.x].y, lat = fin - g.a[b_ + id];
+                        const int fin = e.y + (REC4 ? g.o[b_ + id] : qrec[e.x].y), lat = fin - g.a[b_ + id];
                         if (io_.start) io_.start[b_ + id] = e.y;
                         if (io_.finish) io_.finish[b_ + id] = fin;
                         if (io_.p99) io_.lat[b_ + id] = (uint32_t)lat;
@@ -578,10 +614,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         if (!arrived) {
 #pragma unroll
                             for (int w = 0; w < QW; ++w)
-                                asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(w * 32 + lane) * 4u), "r"(qword[w]) : "memory");
+                                asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u), "r"(qword[w]) : "memory");
                             __syncwarp();
                         }
-                        if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(rw >> 5) * 4u), "r"(1u << (rw & 31)) : "memory");
+                        if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(rw >> 5) * 4u), "r"(1u << (rw & 31)) : "memory");
                     } else {
                         // nobody may still be reading the bitmap for the previous step
                         if (!arrived) G::sync();
@@ -615,7 +651,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         __syncwarp();
 #pragma unroll
                         for (int w = 0; w < QW; ++w)
-                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(qword[w]) : "r"(sm32 + (uint32_t)(QRANKS * 8) + (uint32_t)(w * 32 + lane) * 4u) : "memory");
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(qword[w]) : "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u) : "memory");
                         const int r0 = queue_head(hrest, hbase);      // (arrivals set bits: the queue is not empty)
                         if (r0 != head.r) {
                             const int2 v = lds_rec(r0);
@@ -729,13 +765,20 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                             peak = p2 > peak ? p2 : peak;
                         }
                         if (QREG) {
+                            if constexpr (QW <= 2) {
 #pragma unroll
-                            for (int w = 0; w < QW; ++w) {
-                                const uint32_t hb = (uint32_t)head.r - (uint32_t)((w * 32 + lane) << 5);
-                                if (hb < 32u) qword[w] &= ~(1u << hb);
+                                for (int w = 0; w < QW; ++w) {
+                                    const uint32_t hb = (uint32_t)head.r - (uint32_t)((w * 32 + lane) << 5);
+                                    if (hb < 32u) qword[w] &= ~(1u << hb);
+                                }
+                            } else {          // many words: one mask, applied to the head's word only
+                                const int wi = head.r >> 10;
+                                const uint32_t m = lane == ((head.r >> 5) & 31) ? ~(1u << (head.r & 31)) : ~0u;
+#pragma unroll
+                                for (int w = 0; w < QW; ++w) if (w == wi) qword[w] &= m;
                             }
                             // every lane, same value: one broadcast store
-                            asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)(QRANKS * 8 + 32 * QW * 4) + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
+                            asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)OFF_OBUF + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
                             if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }

@@ -426,16 +426,18 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     c.gslot_bytes = 0; c.max_cta_per_sm = 2;
     if (c.slots) {
         auto ext_of = [&](int th) { int64_t e = mx - (int64_t)th * c.k; e = e > 0 ? (e + 3) / 4 * 4 : 0; return (int)e; };
-        c.qreg = threads == 32 && c.k == SLOT_K && mx <= QREG_RANKS * QREG_MAX_WORDS;
+        // the register queue: instances up to 2,048 requests with 8-byte records (16 slots per thread);
+        // up to 8,192 requests with packed records (16 or 32 slots per thread)
+        c.qreg = threads == 32 && (c.k == SLOT_K ? mx <= QREG_RANKS * QREG_MAX_WORDS : (mx > 2 * QREG_RANKS && mx <= QREG_RANKS * QREG_MAX_WORDS));
         if (c.qreg) {
             // records + bitmap mirror in shared memory, ext slots in a global slot per CTA
-            c.qw = mx <= QREG_RANKS ? 1 : 2;
+            c.qw = mx <= QREG_RANKS ? 1 : (mx <= 2 * QREG_RANKS ? 2 : QREG_MAX_WORDS);
             c.qcap = 0;
             c.ecap = ext_of(32);
-            c.state_bytes = qreg_smem_bytes(c.qw);
+            c.state_bytes = qreg_smem_bytes(c.qw, c.qw > 2);
             c.smem = true;
             c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
-            c.max_cta_per_sm = 32;
+            c.max_cta_per_sm = c.qw > 2 ? 8 : 32;
         } else if (threads == 32 && slot_state_bytes(c.qcap, ext_of(32)) > SMEM_WARP_STATE_LIMIT &&
                    slot_state_bytes(c.qcap, 0) <= SMEM_WARP_STATE_LIMIT) {
             // one warp per item, more than 1024 requests per instance: the bitmaps stay in shared
@@ -479,12 +481,13 @@ int sim_grid(const SimConfig& c, int64_t I)
 template <int THREADS, bool SMEM, bool QREG, int QW = 1, int KS = SLOT_K>
 int slots_grid(const SimConfig& c, int64_t I)
 {
+    constexpr bool REC4 = QW > 2;
     int per_sm = 0;
     if (SMEM) {
-        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, false, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
-        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, true, QREG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, false, QREG, QW, REC4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
+        cudaFuncSetAttribute(k_sim_slots<THREADS, KS, SMEM, true, QREG, QW, REC4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.dyn_smem);
     }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, KS, SMEM, false, QREG, QW>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sim_slots<THREADS, KS, SMEM, false, QREG, QW, REC4>, THREADS, c.dyn_smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
     int64_t grid = (int64_t)per_sm * sm_count();
     if (grid > I) grid = I;
@@ -495,6 +498,7 @@ int slots_grid(const SimConfig& c, int64_t I)
 int sim_grid_any(const SimConfig& c, int64_t I)
 {
     if (c.slots) {
+        if (c.qreg && c.qw > 2) return c.k == 32 ? slots_grid<32, true, true, QREG_MAX_WORDS, 32>(c, I) : slots_grid<32, true, true, QREG_MAX_WORDS>(c, I);
         if (c.qreg) return c.qw == 2 ? slots_grid<32, true, true, 2>(c, I) : slots_grid<32, true, true, 1>(c, I);
         if (c.k == 32) return slots_grid<32, true, false, 1, 32>(c, I);
         if (c.smem) {
@@ -760,7 +764,14 @@ int simulate_impl(const svf_trace_t* tr, int P, const int* policies, int64_t M, 
         if (count) k_sim_slots<T, SLOT_K, S, true, Q, ##__VA_ARGS__><<<grid, T, c.dyn_smem, st>>>(q);   \
         else       k_sim_slots<T, SLOT_K, S, false, Q, ##__VA_ARGS__><<<grid, T, c.dyn_smem, st>>>(q);  \
     } while (0)
-    if (c.qreg) {
+    if (c.qreg && c.qw > 2) {
+        if (c.k == 32) {
+            if (count) k_sim_slots<32, 32, true, true, true, QREG_MAX_WORDS, true><<<grid, 32, c.dyn_smem, st>>>(q);
+            else       k_sim_slots<32, 32, true, false, true, QREG_MAX_WORDS, true><<<grid, 32, c.dyn_smem, st>>>(q);
+        } else {
+            SVF_SLOTS_LAUNCH(32, true, true, QREG_MAX_WORDS, true);
+        }
+    } else if (c.qreg) {
         if (c.qw == 2) SVF_SLOTS_LAUNCH(32, true, true, 2);
         else           SVF_SLOTS_LAUNCH(32, true, true, 1);
     } else if (c.k == 32) {

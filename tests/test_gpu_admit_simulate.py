@@ -224,7 +224,7 @@ def test_group_widths_and_state_placement(B, oracle):
     """Shapes that select each form of the one-warp kernel (M = 60,000: few requests run at once); the
     CTA-wide kernels and the 32-slot warp kernel are in the crowd test, configs[3] and configs[4]."""
     shapes = [(200, 1300, 4.0),        # one warp each, two bitmap words per lane (more than 1024 requests)
-              (100, 2500, 8.0),        # one warp each, shared-memory bitmap (more than 2048 requests)
+              (100, 2500, 8.0),        # one warp each, register queue of eight words per lane, packed records (2,049 .. 8,192 requests)
               (4096 // 8, 40, 2.0),     # many small instances -> one warp each
               (100, 600, 4.0),         # register queue, one bitmap word per lane
               (1, 2000, 4.0),          # a single instance: register queue, two words per lane
@@ -494,6 +494,26 @@ def test_stochastic_reference_workload(B, oracle):
         tr = T.stochastic(n_instances=48, n=600, lam=lam, M=M)
         for policy in range(4):
             check(B, oracle, tr, policy, ctx=f"{tr.name} M={M} policy {policy}")
+
+
+def test_packed_waiting_records_and_their_fallback(B, oracle):
+    """Instances of 2,049 .. 8,192 requests take the register queue with (s, o) packed into ONE word per
+    rank, the split chosen per instance from the widths of its largest s and o; an instance whose
+    widths do not fit 32 bits together (here 18 + 17) reads its records from global memory instead.
+    Both in one call, under 16 (M = 200k) and 32 (M = 600k) register slots per thread."""
+    def inst(j, n, wide):
+        tr = T.config2(instance=300 + j, n=n, lam=6.0)
+        s, o = tr.prompt.copy(), tr.output.copy()
+        if wide:
+            s[7], o[7] = 1 << 17, 3
+            s[11], o[11] = 5, 1 << 16
+        return T._one("", tr.arrival, s, o, (o > 256).astype(np.uint8), 0, 113, 572)
+    for M in (200_000, 600_000):
+        tr = T.concat([inst(0, 2100, False), inst(1, 3000, True), inst(2, 2049, True), inst(3, 5000, False)],
+                      f"packed M={M}", M, 113, 572)
+        for policy in (0, 1, 2, 3):
+            ref, _ = check(B, oracle, tr, policy, ctx=f"{tr.name} policy {policy}")
+            assert not ref.status.any()
 
 
 def test_more_running_requests_than_register_slots(B, oracle):
