@@ -369,6 +369,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     __shared__ int scratch[2][64];
     __shared__ int red[2][WARPS][3];
     __shared__ long long inst_s;
+    __shared__ __align__(16) int4 pre_s[2][WARPS];      // non-QREG: prefetched record of the second waiting request, per warp
     // the p99 selection's histogram: its own kilobyte, except under QREG where it reuses the (s, o)
     // records (dead once the instance is simulated; one kilobyte less per CTA = one more CTA per SM)
     __shared__ uint32_t hist_s[QREG ? 1 : 256];
@@ -593,6 +594,13 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             G::sync();
 
             Rec head, second;
+            // non-QREG: the record of `second` is prefetched by an ASYNCHRONOUS copy into a 16-byte slot of
+            // shared memory per warp (cp.async: no register, no scoreboard) and read at the next promotion,
+            // one evaluation later; sec_pend: the record of `second` is in that slot, not in registers.
+            // (Prefetched into registers, ptxas settles the load's scoreboard at the loop header: the warp
+            // waited there for the L2 round trip, 11 % of the stall samples of configs[3].)
+            bool sec_pend = false;
+            int pre_par = 0;
             head.r = INT_MAX; head.s = head.o = head.id = head.a = 0;
             second = head;
             int next = 0, started = 0, hw = 0;
@@ -634,10 +642,12 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                 } else {
                                     second = head;
                                 }
+                                sec_pend = false;
                                 head = n1;
                                 t_lb = t;                 // a new head: evaluate it now
                             } else {
                                 second = win_rec(l1, r1);
+                                sec_pend = false;
                             }
                         }
                     }
@@ -802,12 +812,21 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         } else {
                             // promote the second; fetch the record behind it one admission ahead
                             head = second;
+                            if (sec_pend) {
+                                asm volatile("cp.async.wait_all;" ::: "memory");
+                                __syncwarp();
+                                const int4 qv = pre_s[pre_par][wrp];
+                                head.s = qv.x; head.o = qv.y; head.id = qv.z; head.a = qv.w;
+                            }
                             second.r = INT_MAX;
                             if (head.r == INT_MAX) break;
                             const int r = queue_first_ge(L0, L1, n, nL1, head.r + 1);
                             if (r != INT_MAX) {
-                                const int4 qv = req[r];
-                                second.r = r; second.s = qv.x; second.o = qv.y; second.id = qv.z; second.a = qv.w;
+                                second.r = r;
+                                sec_pend = true;
+                                pre_par ^= 1;                 // (the slot just read is not overwritten while a lane may still read it)
+                                if (lane == 0)
+                                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((uint32_t)__cvta_generic_to_shared(&pre_s[pre_par][wrp])), "l"(req + r) : "memory");
                             }
                         }
                     }

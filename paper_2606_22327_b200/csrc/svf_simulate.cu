@@ -453,7 +453,16 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
             c.ecap = ext_of(threads);
             c.state_bytes = slot_state_bytes(c.qcap, c.ecap);
             c.smem = c.state_bytes <= (threads == 32 ? SMEM_WARP_STATE_LIMIT : SMEM_STATE_LIMIT);
-            if (!c.smem) c.gslot_bytes = align_up(c.state_bytes, 256);
+            if (!c.smem && threads > 32 && slot_state_bytes(c.qcap, 0) <= SMEM_STATE_LIMIT) {
+                // a CTA-wide group whose ext slots outgrow shared memory (configs[3]: 2.4 MB of them, hardly
+                // ever touched): the two-level bitmap (searched after every admission) stays in shared
+                // memory, only the ext slots go to the global slot
+                c.state_bytes = slot_state_bytes(c.qcap, 0);
+                c.smem = true; c.ext_global = true;
+                c.gslot_bytes = align_up(qreg_ext_bytes(c.ecap), 256);
+            } else if (!c.smem) {
+                c.gslot_bytes = align_up(c.state_bytes, 256);
+            }
         }
     } else {
         c.state_bytes = state_bytes(c.cap);
