@@ -277,10 +277,21 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     case 4: OP(4) break; case 5: OP(5) break; case 6: OP(6) break; case 7: OP(7) break; case 8: OP(8) break; case 9: OP(9) break; \
     case 10: OP(10) break; case 11: OP(11) break; case 12: OP(12) break; case 13: OP(13) break; case 14: OP(14) break; default: OP(15) break; }
 #else
+// (two levels of uniform branches, then the four slots of the group under predicates: a quarter of the
+// code of the full tree)
+#define SVF_PUTG(ik, k0)  { const int j_ = (ik) & 3;                                          \
+    if (mine && j_ == 0) { f[k0] = fh; B[k0] = Bh; c[k0] = add; }                                 \
+    if (mine && j_ == 1) { f[k0 + 1] = fh; B[k0 + 1] = Bh; c[k0 + 1] = add; }                     \
+    if (mine && j_ == 2) { f[k0 + 2] = fh; B[k0 + 2] = Bh; c[k0 + 2] = add; }                     \
+    if (mine && j_ == 3) { f[k0 + 3] = fh; B[k0 + 3] = Bh; c[k0 + 3] = add; } }
+#define SVF_PUT16G(ik)        if ((ik) & 8) { if ((ik) & 4) SVF_PUTG(ik, 12) else SVF_PUTG(ik, 8) } else { if ((ik) & 4) SVF_PUTG(ik, 4) else SVF_PUTG(ik, 0) }
 #define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
 #endif
 #define SVF_PUT32(ik, OP)     if ((ik) & 16) { if ((ik) & 8) { SVF_PUT8(ik, OP, 24) } else { SVF_PUT8(ik, OP, 16) } } else { SVF_PUT16(ik, OP) }
-#define SVF_PUTK(ik, OP)      if constexpr (K == 32) { SVF_PUT32(ik, OP) } else { SVF_PUT16(ik, OP) }
+#define SVF_PUT32G(ik)        if ((ik) & 16) { if ((ik) & 8) { if ((ik) & 4) SVF_PUTG(ik, 28) else SVF_PUTG(ik, 24) } else { if ((ik) & 4) SVF_PUTG(ik, 20) else SVF_PUTG(ik, 16) } } else { SVF_PUT16G(ik) }
+// LAT (kernels that run as a few lone groups: latency matters, not the instruction count): the compact form
+#define SVF_PUTK(ik, OP)      if constexpr (LAT) { if constexpr (K == 32) { SVF_PUT32G(ik) } else { SVF_PUT16G(ik) } }        \
+                              else if constexpr (K == 32) { SVF_PUT32(ik, OP) } else { SVF_PUT16(ik, OP) }
 
 // The per-slot operations of the passes.  They are macros over the LOCAL names of the calling
 // kernel (k_sim_slots here, k_admit_slots in svf_admit.cu): slots f[], B[], c[]; the head's t1 =
@@ -356,6 +367,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     static_assert(QW >= 1 && QW <= QREG_MAX_WORDS && (QREG || QW == 1), "QW: bitmap words per lane of the register queue");
     static_assert(!REC4 || QREG, "REC4: packed records of the register queue");
     constexpr int QRANKS = QREG_RANKS * QW;
+    // the bench-shaped kernel (thousands of one-warp items: 20 warps per SM share the issue ports) is tuned
+    // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
+    // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
+    constexpr bool LAT = !(QREG && QW == 1);
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
     constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
