@@ -567,3 +567,28 @@ def test_fuzz_random_batches(B, oracle, rnd):
     for pol, out in zip(pols, outs):
         ref = oracle.simulate(tr, pol, n_threads=8)
         assert_same({k: getattr(out, k).cpu().numpy() for k in FIELDS}, ref, tr, f"fuzz {rnd} policy {pol}")
+
+
+@pytest.mark.parametrize("rnd", range(3))
+def test_fuzz_packed_register_queue(B, oracle, rnd):
+    """The same over the sizes of the packed register queue (instances up to 8,192 requests): ragged
+    sizes, budgets from a handful to hundreds of running requests (16 and 32 slots per thread, ext
+    slots), bursts and spread arrivals, two policies per call."""
+    sd = T.instance_seed(57, rnd)
+    u = lambda stream, lo, hi: int(T.uniform_int(sd, stream, 1, lo, hi)[0])
+    s_hi, o_hi = u(1, 20, 400), u(2, 20, 600)
+    M = u(3, 4 * (s_hi + o_hi), (20, 300, 900)[rnd] * (s_hi + o_hi))
+    parts = []
+    for i in range(10):
+        si = T.instance_seed(58, rnd * 1000 + i)
+        n = int(T.uniform_int(si, 1, 1, 0, 8192)[0]) if i else 8192
+        a_hi = (0, 30, 3000)[int(T.uniform_int(si, 2, 1, 0, 2)[0])]
+        parts.append(T.random_small(rnd * 1000 + i + 77, n, s_hi, o_hi, M, a_hi=a_hi, O0=3, O1=40))
+    tr = T.concat(parts, f"fuzz-packed{rnd}", M, 3, 40)
+    pols = [rnd % 4, (rnd + 1) % 4]
+    import torch
+    outs = B.svf_simulate_policies(B.DeviceTrace.from_host(tr), pols)
+    torch.cuda.synchronize()
+    for pol, out in zip(pols, outs):
+        ref = oracle.simulate(tr, pol, n_threads=8)
+        assert_same({k: getattr(out, k).cpu().numpy() for k in FIELDS}, ref, tr, f"fuzz-packed {rnd} policy {pol}")
