@@ -263,7 +263,15 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     if ((g4) >= 6) { OP(23) OP(22) OP(21) OP(20) }                                            \
     if ((g4) >= 5) { OP(19) OP(18) OP(17) OP(16) }                                            \
     SVF_SLOT_GROUPS(g4, OP)
-#define SVF_SLOTS(g4, OP) if constexpr (K == 32) { SVF_SLOT_GROUPS32(g4, OP) } else { SVF_SLOT_GROUPS(g4, OP) }
+// LAT (a few lone groups per SM): eight slots per basic block -- more independent chains for the one warp
+// that has a scheduler to itself, half the branches; the bench-shaped kernel keeps groups of four
+#define SVF_SLOT_GROUPS_8(g4, OP)                                                             \
+    if ((g4) >= 3) { OP(15) OP(14) OP(13) OP(12) OP(11) OP(10) OP(9) OP(8) OP(7) OP(6) OP(5) OP(4) OP(3) OP(2) OP(1) OP(0) }  \
+    else if ((g4) >= 1) { OP(7)  OP(6)  OP(5)  OP(4)  OP(3)  OP(2)  OP(1) OP(0) }
+#define SVF_SLOT_GROUPS32_16(g4, OP)                                                          \
+    if ((g4) >= 5) { OP(31) OP(30) OP(29) OP(28) OP(27) OP(26) OP(25) OP(24) OP(23) OP(22) OP(21) OP(20) OP(19) OP(18) OP(17) OP(16) }  \
+    SVF_SLOT_GROUPS_8(g4, OP)
+#define SVF_SLOTS(g4, OP) if constexpr (K == 32) { SVF_SLOT_GROUPS32_16(g4, OP) } else if constexpr (LAT8) { SVF_SLOT_GROUPS_8(g4, OP) } else { SVF_SLOT_GROUPS(g4, OP) }
 
 // write into register slot ik (uniform) of the owning thread: a tree of uniform branches
 #define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
@@ -371,6 +379,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
+    constexpr bool LAT8 = LAT && K == 16;
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
     constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
