@@ -263,8 +263,10 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     if ((g4) >= 6) { OP(23) OP(22) OP(21) OP(20) }                                            \
     if ((g4) >= 5) { OP(19) OP(18) OP(17) OP(16) }                                            \
     SVF_SLOT_GROUPS(g4, OP)
-// LAT (a few lone groups per SM): eight slots per basic block -- more independent chains for the one warp
-// that has a scheduler to itself, half the branches; the bench-shaped kernel keeps groups of four
+// sixteen slots in ONE basic block while more than eight slots per thread are in use, else eight (g4 is 4 or
+// 2 here, see the pass): more independent chains per block, a fifth of the branches, half the code of one
+// block per group of four -- measured on the bench kernel: 6.12 -> 6.05 ms (one block per group count
+// 6.08, always sixteen 6.11, eight + eight 6.06), on a lone warp (configs[1]) 1.49 -> 1.39 ms
 #define SVF_SLOT_GROUPS_8(g4, OP)                                                             \
     if ((g4) >= 3) { OP(15) OP(14) OP(13) OP(12) OP(11) OP(10) OP(9) OP(8) OP(7) OP(6) OP(5) OP(4) OP(3) OP(2) OP(1) OP(0) }  \
     else if ((g4) >= 1) { OP(7)  OP(6)  OP(5)  OP(4)  OP(3)  OP(2)  OP(1) OP(0) }
@@ -379,7 +381,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
-    constexpr bool LAT8 = LAT && K == 16;
+    constexpr bool LAT8 = K == 16;
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
     constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
@@ -708,8 +710,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         const uint32_t add = (uint32_t)head.s - (uint32_t)t;                  // A_j += s_h - t + f_j
                         uint32_t acc = 0, acc1 = 0, dm = 0;
                         int viol = INT_MIN;
-                        int kmax = (hw + THREADS - 1) >> TSHIFT; kmax = kmax < K ? kmax : K;   // register slots in use per thread
-                        const int g4 = (kmax + 3) >> 2;
+                        // groups of four register slots processed per thread: 2 (eight slots), 4 (sixteen) or 8
+                        // (thirty-two); slots past the high-water mark are dead (f = 0) and cost their instructions only
+                        const int g4 = (K == 32 && hw > 16 * THREADS) ? 8 : (hw > 8 * THREADS ? 4 : 2);
                         const bool use_ext = hw > REGCAP;
                         SVF_SLOTS(g4, SVF_EVAL)
                         // lowest free register slot of this thread as a one-hot bit (bit k of dm =
