@@ -382,6 +382,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
     constexpr bool LAT8 = K == 16;
+    // (rank, start) of the last <= 32 admissions: two registers per lane where registers are free (configs[1]
+    // 1.34 -> 1.32 ms), the shared-memory buffer in the bench-shaped kernel (at its 96 registers: 5.80 against 5.95 ms)
+    constexpr bool OBUF_REG = QREG && LAT;
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
     constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
@@ -538,7 +541,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 #pragma unroll
             for (int w = 0; w < QW; ++w) qword[w] = 0;
             // lowest waiting rank (INT_MAX if none), the rest of its word above it, the word's first rank
-            auto queue_head = [&](uint32_t& rest, int& wbase_) -> int {
+            auto queue_head = [&](uint32_t& rest, int& wbase_, uint32_t& bit_) -> int {
 #pragma unroll
                 for (int w = 0; w < QW; ++w) {
                     const uint32_t nz = __ballot_sync(FULL, qword[w] != 0u);
@@ -546,8 +549,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         const int l0 = __ffs(nz) - 1;
                         const uint32_t w0 = __shfl_sync(FULL, qword[w], l0);
                         wbase_ = (w * 32 + l0) * 32;
-                        rest = w0 & (w0 - 1u);
-                        return wbase_ + (__ffs(w0) - 1);
+                        bit_ = w0 & (0u - w0);
+                        rest = w0 ^ bit_;
+                        return wbase_ + (31 - __clz(bit_));
                     }
                 }
                 return INT_MAX;
@@ -598,7 +602,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         int pi_ = pi; long long b_ = base;
                         asm volatile("" : "+r"(pi_), "+l"(b_));
                         const PolicyIO& io_ = g.io[pi_];
-                        const int2 e = obuf[lane];
+                        const int2 e = OBUF_REG ? make_int2(b_id, b_t) : obuf[lane];
                         const int id = (int)io_.order[b_ + e.x];
                         const int fin = e.y + (REC4 ? g.o[b_ + id] : qrec[e.x].y), lat = fin - g.a[b_ + id];
                         if (io_.start) io_.start[b_ + id] = e.y;
@@ -630,7 +634,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             head.r = INT_MAX; head.s = head.o = head.id = head.a = 0;
             second = head;
             int next = 0, started = 0, hw = 0;
-            uint32_t hrest = 0; int hbase = 0;    // QREG: the head's bitmap word above the head, and its first rank
+            uint32_t hrest = 0, hbit = 0; int hbase = 0;    // QREG: the head's bitmap word above the head, the head's own bit in it (one-hot), the word's first rank
             int32_t t = a[0];
             int32_t t_lb = t;                     // first step at which the head must be (re)evaluated
 
@@ -688,7 +692,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 #pragma unroll
                         for (int w = 0; w < QW; ++w)
                             asm volatile("ld.shared.u32 %0, [%1];" : "=r"(qword[w]) : "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u) : "memory");
-                        const int r0 = queue_head(hrest, hbase);      // (arrivals set bits: the queue is not empty)
+                        const int r0 = queue_head(hrest, hbase, hbit);      // (arrivals set bits: the queue is not empty)
                         if (r0 != head.r) {
                             const int2 v = lds_rec(r0);
                             head.r = r0; head.s = v.x; head.o = v.y;
@@ -722,9 +726,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         if constexpr (K == 32) {      // 32 slots: the key carries the slot NUMBER (32 = none)
                             const uint32_t dmx = dm | (g4 < 8 ? (1u << (4 * g4)) : 0u);
                             fkey = ((dmx ? __ffs(dmx) - 1 : K) << TSHIFT) | tid;
-                        } else {
+                        } else {       // (the sentinel keeps dmx non-zero; slot 16 = none)
                             const uint32_t dmx = dm | (1u << (4 * g4));
-                            fkey = (int)(((dmx & (0u - dmx)) << TSHIFT) | (uint32_t)tid);
+                            fkey = ((__ffs(dmx) - 1) << TSHIFT) | tid;
                         }
                         int eidx = INT_MAX;
                         if (use_ext) {
@@ -778,8 +782,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         // ---- admitted: the update is already in place; write the head into a slot --
                         const uint32_t Bh = (uint32_t)Ah + fhu;
                         int idx;
-                        if (K == 32 ? fkey < (K << TSHIFT) : fkey < (1 << (K + TSHIFT))) {
-                            const int ik = K == 32 ? (fkey >> TSHIFT) : 31 - __clz(fkey >> TSHIFT);           // uniform
+                        if (fkey < (K << TSHIFT)) {
+                            const int ik = fkey >> TSHIFT;           // uniform
                             const bool mine = (fkey & (THREADS - 1)) == tid;
                             idx = (ik << TSHIFT) + (fkey & (THREADS - 1));
                             SVF_PUTK(ik, SVF_PUT)
@@ -804,18 +808,17 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         if (QREG) {
                             if constexpr (QW <= 2) {
 #pragma unroll
-                                for (int w = 0; w < QW; ++w) {
-                                    const uint32_t hb = (uint32_t)head.r - (uint32_t)((w * 32 + lane) << 5);
-                                    if (hb < 32u) qword[w] &= ~(1u << hb);
-                                }
+                                for (int w = 0; w < QW; ++w)      // the head's bit (a uniform one-hot word) leaves its lane's word
+                                    if (w * 32 + lane == (hbase >> 5)) qword[w] ^= hbit;
                             } else {          // many words: one mask, applied to the head's word only
                                 const int wi = head.r >> 10;
                                 const uint32_t m = lane == ((head.r >> 5) & 31) ? ~(1u << (head.r & 31)) : ~0u;
 #pragma unroll
                                 for (int w = 0; w < QW; ++w) if (w == wi) qword[w] &= m;
                             }
-                            // every lane, same value: one broadcast store
-                            asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)OFF_OBUF + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
+                            // the admission goes to lane (started % 32): two registers per lane, written under one predicate
+                            if constexpr (OBUF_REG) { if (lane == (started & 31)) { b_id = head.r; b_t = t; } }
+                            else asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)OFF_OBUF + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
                             if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
@@ -828,10 +831,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                             // from shared memory
                             int r;
                             if (hrest) {
-                                r = hbase + (__ffs(hrest) - 1);
-                                hrest &= hrest - 1u;
+                                hbit = hrest & (0u - hrest);
+                                hrest ^= hbit;
+                                r = hbase + (31 - __clz(hbit));
                             } else {
-                                r = queue_head(hrest, hbase);
+                                r = queue_head(hrest, hbase, hbit);
                                 if (r == INT_MAX) { head.r = INT_MAX; break; }
                             }
                             const int2 v = lds_rec(r);
