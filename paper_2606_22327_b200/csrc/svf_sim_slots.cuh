@@ -245,35 +245,26 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     return prefix;
 }
 
-// straight-line code over register slots 4*g4-1 .. 0 (g4 = groups of four slots in use): at most
-// four uniform compare-and-branch, no indexed branch, no loop overhead; four slots per basic
-// block so that the compiler can interleave their dependent chains (x -> compare -> predicated
-// op).  A slot past the high-water mark is dead (f = 0) and costs its instructions only.
+// The slot passes are straight-line code over the register slots, no loop, no indexed branch.  A slot past
+// the high-water mark is dead (f = 0) and costs its instructions only.
+// k_admit_slots (svf_admit.cu): groups of four slots behind a ladder of uniform compares (g4 = groups in use)
 #define SVF_SLOT_GROUPS(g4, OP)                                                               \
     if ((g4) >= 4) { OP(15) OP(14) OP(13) OP(12) }                                            \
     if ((g4) >= 3) { OP(11) OP(10) OP(9)  OP(8)  }                                            \
     if ((g4) >= 2) { OP(7)  OP(6)  OP(5)  OP(4)  }                                            \
     if ((g4) >= 1) { OP(3)  OP(2)  OP(1)  OP(0)  }
-
-// the same for 32 register slots per thread (K = 32: 1,024 slots on one warp, for running sets that
-// outgrow 512 where a CTA-wide group would replicate the scalar part in every warp)
-#define SVF_SLOT_GROUPS32(g4, OP)                                                             \
-    if ((g4) >= 8) { OP(31) OP(30) OP(29) OP(28) }                                            \
-    if ((g4) >= 7) { OP(27) OP(26) OP(25) OP(24) }                                            \
-    if ((g4) >= 6) { OP(23) OP(22) OP(21) OP(20) }                                            \
-    if ((g4) >= 5) { OP(19) OP(18) OP(17) OP(16) }                                            \
-    SVF_SLOT_GROUPS(g4, OP)
-// sixteen slots in ONE basic block while more than eight slots per thread are in use, else eight (g4 is 4 or
-// 2 here, see the pass): more independent chains per block, a fifth of the branches, half the code of one
-// block per group of four -- measured on the bench kernel: 6.12 -> 6.05 ms (one block per group count
-// 6.08, always sixteen 6.11, eight + eight 6.06), on a lone warp (configs[1]) 1.49 -> 1.39 ms
+// k_sim_slots: sixteen slots in ONE basic block while more than eight slots per thread are in use, else eight
+// (g4 is 4 or 2 here -- 8 with 32 slots per thread: sixteen more in a block of their own --, see the pass):
+// sixteen independent chains per block, a fifth of the branches, half the code of one block per group of
+// four -- measured on the bench kernel: 6.12 -> 6.05 ms (one block per group count 6.08, always sixteen
+// 6.11, eight + eight 6.06), with the one-compare block choice 5.89; on a lone warp (configs[1]) 1.49 -> 1.34 ms
 #define SVF_SLOT_GROUPS_8(g4, OP)                                                             \
     if ((g4) >= 3) { OP(15) OP(14) OP(13) OP(12) OP(11) OP(10) OP(9) OP(8) OP(7) OP(6) OP(5) OP(4) OP(3) OP(2) OP(1) OP(0) }  \
     else if ((g4) >= 1) { OP(7)  OP(6)  OP(5)  OP(4)  OP(3)  OP(2)  OP(1) OP(0) }
 #define SVF_SLOT_GROUPS32_16(g4, OP)                                                          \
     if ((g4) >= 5) { OP(31) OP(30) OP(29) OP(28) OP(27) OP(26) OP(25) OP(24) OP(23) OP(22) OP(21) OP(20) OP(19) OP(18) OP(17) OP(16) }  \
     SVF_SLOT_GROUPS_8(g4, OP)
-#define SVF_SLOTS(g4, OP) if constexpr (K == 32) { SVF_SLOT_GROUPS32_16(g4, OP) } else if constexpr (LAT8) { SVF_SLOT_GROUPS_8(g4, OP) } else { SVF_SLOT_GROUPS(g4, OP) }
+#define SVF_SLOTS(g4, OP) if constexpr (K == 32) { SVF_SLOT_GROUPS32_16(g4, OP) } else { SVF_SLOT_GROUPS_8(g4, OP) }
 
 // write into register slot ik (uniform) of the owning thread: a tree of uniform branches
 #define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
@@ -381,7 +372,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
-    constexpr bool LAT8 = K == 16;
     // (rank, start) of the last <= 32 admissions: two registers per lane where registers are free (configs[1]
     // 1.34 -> 1.32 ms), the shared-memory buffer in the bench-shaped kernel (at its 96 registers: 5.80 against 5.95 ms)
     constexpr bool OBUF_REG = QREG && LAT;
