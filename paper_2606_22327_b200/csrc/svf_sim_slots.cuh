@@ -205,13 +205,15 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     using G = Group<THREADS>;
     const int tid = threadIdx.x, lane = tid & 31;
     uint32_t vor = 0;
+#pragma unroll 8
     for (int i = tid; i < n; i += THREADS) vor |= __ldcg(v + i);
     vor = G::or_u32(vor, scratch, parity);
     uint32_t prefix = 0, pmask = 0;
     for (int shift = vor ? ((31 - __clz(vor)) & ~7) : 0; shift >= 0; shift -= 8) {
         for (int i = tid; i < 256; i += THREADS) hist[i] = 0;
         G::sync();
-        for (int i = tid; i < n; i += THREADS) {
+#pragma unroll 8
+        for (int i = tid; i < n; i += THREADS) {       // (unrolled: eight L2 loads in flight per thread)
             const uint32_t x = __ldcg(v + i);
             if ((x & pmask) == prefix) atomicAdd(&hist[(x >> shift) & 255u], 1u);
         }
