@@ -199,14 +199,16 @@ __device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, 
 // uniform.  One 256-bin histogram in shared memory per significant byte; v was written by this
 // group before a barrier (read with ld.cg, never through the non-coherent path).
 template <int THREADS>
+// (sub != NULL: the values are v[i] - sub[i]: the register-queue kernels store finish times and take the
+// arrivals off here, in index order, instead of gathering a[id] in the output flush)
 __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, int k, uint32_t* hist,
-                                                     int (*scratch)[64], int& parity)
+                                                     int (*scratch)[64], int& parity, const int32_t* sub = nullptr)
 {
     using G = Group<THREADS>;
     const int tid = threadIdx.x, lane = tid & 31;
     uint32_t vor = 0;
 #pragma unroll 8
-    for (int i = tid; i < n; i += THREADS) vor |= __ldcg(v + i);
+    for (int i = tid; i < n; i += THREADS) vor |= __ldcg(v + i) - (sub ? (uint32_t)sub[i] : 0u);
     vor = G::or_u32(vor, scratch, parity);
     uint32_t prefix = 0, pmask = 0;
     for (int shift = vor ? ((31 - __clz(vor)) & ~7) : 0; shift >= 0; shift -= 8) {
@@ -214,7 +216,7 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
         G::sync();
 #pragma unroll 8
         for (int i = tid; i < n; i += THREADS) {       // (unrolled: eight L2 loads in flight per thread)
-            const uint32_t x = __ldcg(v + i);
+            const uint32_t x = __ldcg(v + i) - (sub ? (uint32_t)sub[i] : 0u);
             if ((x & pmask) == prefix) atomicAdd(&hist[(x >> shift) & 255u], 1u);
         }
         G::sync();
@@ -453,7 +455,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
         const int32_t* __restrict__ o = g.o + base;
 
         // ---- validation (data errors -> status[j], never UB) --------------------------------
-        int64_t sum_o = 0;
+        int64_t sum_o = 0, sum_a = 0;
         int max_a = 0, max_s = 0, max_o = 0;
         // (unrolled: the loads of several rounds in flight; the loop is 4 % of the stall samples of the bench kernel)
 #pragma unroll (LAT ? 8 : 4)
@@ -466,6 +468,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
             if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
+            if (QREG) sum_a += ai;
             max_a = ai > max_a ? ai : max_a;
             if (REC4) { max_s = si > max_s ? si : max_s; max_o = oi > max_o ? oi : max_o; }
             // QREG: the (s, o) of every request by RANK in shared memory, once per instance (the presort
@@ -579,7 +582,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 }
             };
             load_window();
-            if (QREG) { tel_s[lane] = 0; mk_s[lane] = 0; }
+            if (QREG) { tel_s[lane] = -sum_a; mk_s[lane] = 0; }     // (the sum of the finish times is added to minus this lane's share of the arrivals)
             auto win_rec = [&](int l, int r) {
                 Rec x; x.r = r; x.s = __shfl_sync(FULL, sw, l); x.o = __shfl_sync(FULL, ow, l);
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
@@ -598,11 +601,13 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         const PolicyIO& io_ = g.io[pi_];
                         const int2 e = OBUF_REG ? make_int2(b_id, b_t) : obuf[lane];
                         const int id = (int)io_.order[b_ + e.x];
-                        const int fin = e.y + (REC4 ? g.o[b_ + id] : qrec[e.x].y), lat = fin - g.a[b_ + id];
+                        // (no a[id] here, a second dependent round trip: the total latency is the sum of the
+                        // finish times minus the sum of the arrivals, and the p99 selection takes the arrivals off)
+                        const int fin = e.y + (REC4 ? g.o[b_ + id] : qrec[e.x].y);
                         if (io_.start) io_.start[b_ + id] = e.y;
                         if (io_.finish) io_.finish[b_ + id] = fin;
-                        if (io_.p99) io_.lat[b_ + id] = (uint32_t)lat;
-                        tel_s[lane] += lat;
+                        if (io_.p99) io_.lat[b_ + id] = (uint32_t)fin;
+                        tel_s[lane] += fin;
                         if (fin > mk_s[lane]) mk_s[lane] = fin;
                     }
                 } else if (wrp == 0 && lane < count) {
@@ -877,7 +882,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             decisions += (uint32_t)started;
             if (want_p99) {                       // nearest rank ceil(0.99 n), 1-based (R13)
                 G::sync();
-                p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity);
+                p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity, QREG ? a : nullptr);
             }
         }
         if (COUNT) {
