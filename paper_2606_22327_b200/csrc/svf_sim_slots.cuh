@@ -455,7 +455,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
         const int32_t* __restrict__ o = g.o + base;
 
         // ---- validation (data errors -> status[j], never UB) --------------------------------
-        int64_t sum_o = 0, sum_a = 0;
+        int64_t sum_o = 0;
         int max_a = 0, max_s = 0, max_o = 0;
         // (unrolled: the loads of several rounds in flight; the loop is 4 % of the stall samples of the bench kernel)
 #pragma unroll (LAT ? 8 : 4)
@@ -468,7 +468,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             const uint32_t b = policy == SVF_SVF_1BIT ? (uint32_t)g.bit[base + i] : 0u;
             if (oi >= 1 && si >= 0 && ai >= 0 && ki >= 1 && (priority_key(policy, si, ki, ai, b, g.O0, g.O1) >> 32)) flags |= F_OVERFLOW;
             sum_o += oi > 0 ? oi : 0;
-            if (QREG) sum_a += ai;
             max_a = ai > max_a ? ai : max_a;
             if (REC4) { max_s = si > max_s ? si : max_s; max_o = oi > max_o ? oi : max_o; }
             // QREG: the (s, o) of every request by RANK in shared memory, once per instance (the presort
@@ -582,7 +581,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 }
             };
             load_window();
-            if (QREG) { tel_s[lane] = -sum_a; mk_s[lane] = 0; }     // (the sum of the finish times is added to minus this lane's share of the arrivals)
             auto win_rec = [&](int l, int r) {
                 Rec x; x.r = r; x.s = __shfl_sync(FULL, sw, l); x.o = __shfl_sync(FULL, ow, l);
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
@@ -593,23 +591,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             // up when the buffer is written)
             int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
             auto flush = [&](int count) {
-                if (QREG) __syncwarp();
                 if (QREG) {
-                    if (lane < count) {
-                        int pi_ = pi; long long b_ = base;
-                        asm volatile("" : "+r"(pi_), "+l"(b_));
-                        const PolicyIO& io_ = g.io[pi_];
-                        const int2 e = OBUF_REG ? make_int2(b_id, b_t) : obuf[lane];
-                        const int id = (int)io_.order[b_ + e.x];
-                        // (no a[id] here, a second dependent round trip: the total latency is the sum of the
-                        // finish times minus the sum of the arrivals, and the p99 selection takes the arrivals off)
-                        const int fin = e.y + (REC4 ? g.o[b_ + id] : qrec[e.x].y);
-                        if (io_.start) io_.start[b_ + id] = e.y;
-                        if (io_.finish) io_.finish[b_ + id] = fin;
-                        if (io_.p99) io_.lat[b_ + id] = (uint32_t)fin;
-                        tel_s[lane] += fin;
-                        if (fin > mk_s[lane]) mk_s[lane] = fin;
-                    }
                 } else if (wrp == 0 && lane < count) {
                     const int id = b_id, lat = b_lat;
                     if (want_start) out_start[id] = b_t;
@@ -618,7 +600,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                     tel += lat;
                     mk = b_f > mk ? b_f : mk;
                 }
-                if (QREG) __syncwarp();
             };
             G::sync();
 
@@ -815,15 +796,15 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 #pragma unroll
                                 for (int w = 0; w < QW; ++w) if (w == wi) qword[w] &= m;
                             }
-                            // the admission goes to lane (started % 32): two registers per lane, written under one predicate
-                            if constexpr (OBUF_REG) { if (lane == (started & 31)) { b_id = head.r; b_t = t; } }
-                            else asm volatile("st.shared.v2.s32 [%0], {%1, %2};" :: "r"(sm32 + (uint32_t)OFF_OBUF + (uint32_t)(started & 31) * 8u), "r"(head.r), "r"(t) : "memory");
+// the start time takes the place of the admitted request's record (its s is not needed again):
+                            // outputs leave the chip at the end of the instance, in index order
+                            asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)head.r * (uint32_t)RB), "r"(t) : "memory");
                         } else {
                             if (tid == 0) queue_clear(L0, L1, head.r);
                             if (lane == (started & 31)) { b_id = head.id; b_t = t; b_f = fh; b_lat = fh - head.a; }
                         }
                         ++started;                                     // (decisions: the admissions are added at the end)
-                        if ((started & 31) == 0) flush(32);
+                        if (!QREG && (started & 31) == 0) flush(32);
                         if (QREG) {
                             // next head: the next set bit of the word the head came from (a uniform copy
                             // of it, `hrest`), else the lowest set bit of the later words; its (s, o) come
@@ -877,12 +858,28 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 if (tn == INT_MAX) break;                     // nothing left that could ever happen (corrupt rank[]): never spin
                 t = tn;
             }
-            flush(started & 31);
-            if (QREG) { tel = tel_s[lane]; mk = mk_s[lane]; }
+            if (!QREG) flush(started & 31);
+            if (QREG) {
+                // outputs of the whole instance in INDEX order (coalesced loads of rank / a / o, coalesced
+                // stores): the start time of request i waits at its rank in shared memory
+                __syncwarp();
+#pragma unroll 4
+                for (int i = lane; i < n; i += 32) {
+                    const int r = (int)rnk[i] & (QRANKS - 1);
+                    int st, oo;
+                    if (REC4) { st = (int)qrec4[r]; oo = o[i]; } else { const int2 v = qrec[r]; st = v.x; oo = v.y; }
+                    const int fin = st + oo, lat = fin - a[i];
+                    if (want_start) out_start[i] = st;
+                    if (want_finish) out_finish[i] = fin;
+                    if (want_p99) out_lat[i] = (uint32_t)lat;
+                    tel += lat;
+                    mk = fin > mk ? fin : mk;
+                }
+            }
             decisions += (uint32_t)started;
             if (want_p99) {                       // nearest rank ceil(0.99 n), 1-based (R13)
                 G::sync();
-                p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity, QREG ? a : nullptr);
+                p99v = (int64_t)group_select_kth<THREADS>(out_lat, n, (int)((99ll * n + 99) / 100), hist, scratch, parity);
             }
         }
         if (COUNT) {
