@@ -55,9 +55,11 @@
 //    priority order in global memory.
 // The head of the queue is cached in registers (non-QREG: also the second, whose record is
 // fetched one admission ahead to hide the L2 latency).  ARRIVALS come from a 32-wide register window over
-// (a, s, o, rank), refilled once per 32 arrivals.  OUTPUTS (start, finish, latency word) are
-// buffered one admission per lane and written 32 at a time; p99 (nearest rank) is a radix selection
-// over the instance's latencies by the same thread group at the end of the instance.
+// (a, s, o, rank), refilled once per 32 arrivals.  OUTPUTS (start, finish, latency word): QREG: the start
+// time of an admitted request replaces its record in shared memory and everything is written at the
+// end of the instance in index order (coalesced); otherwise buffered one admission per lane and written
+// 32 at a time.  p99 (nearest rank) is a radix selection over the instance's latencies by the same
+// thread group at the end of the instance.
 #pragma once
 
 #include <limits.h>
@@ -165,9 +167,9 @@ __host__ __device__ inline size_t slot_state_bytes(int qcap, int ecap)
 // instead of 64 KB per warp, six warps per SM instead of three)
 constexpr int QREG_RANKS = 1024;
 constexpr int QREG_MAX_WORDS = 8;
-__host__ __device__ constexpr size_t qreg_smem_bytes(int qw, bool rec4 = false)      // (s, o) by rank, bitmap mirror, output buffer
+__host__ __device__ constexpr size_t qreg_smem_bytes(int qw, bool rec4 = false)      // (s, o) by rank (the start time once admitted), bitmap mirror
 {
-    return (size_t)QREG_RANKS * qw * (rec4 ? 4 : 8) + (size_t)32 * qw * 4 + 32 * 8 + 32 * 8 + 32 * 4;   // + per-lane latency sums and makespans
+    return (size_t)QREG_RANKS * qw * (rec4 ? 4 : 8) + (size_t)32 * qw * 4;
 }
 constexpr size_t QREG_SMEM_BYTES = qreg_smem_bytes(1);
 __host__ __device__ inline size_t qreg_ext_bytes(int ecap) { return 3 * align_up((size_t)ecap * 4, 16); }
@@ -376,11 +378,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
-    // (rank, start) of the last <= 32 admissions: two registers per lane where registers are free (configs[1]
-    // 1.34 -> 1.32 ms), the shared-memory buffer in the bench-shaped kernel (at its 96 registers: 5.80 against 5.95 ms)
-    constexpr bool OBUF_REG = QREG && LAT;
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
-    constexpr int OFF_BITS = QRANKS * RB, OFF_OBUF = OFF_BITS + 32 * QW * 4, OFF_TEL = OFF_OBUF + 32 * 8, OFF_MK = OFF_TEL + 32 * 8;
+    constexpr int OFF_BITS = QRANKS * RB;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
     static_assert(!QREG || (THREADS == 32 && SMEM), "QREG: one warp per instance, queue records in shared memory");
     using G = Group<THREADS>;
@@ -414,11 +413,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     uint32_t* ec = reinterpret_cast<uint32_t*>(ebase + 2 * estride);
     int2* qrec = reinterpret_cast<int2*>(dyn_smem);                                   // QREG only (REC4: one packed word per rank)
     uint32_t* qrec4 = reinterpret_cast<uint32_t*>(dyn_smem);
-    int2* obuf = reinterpret_cast<int2*>(dyn_smem + OFF_OBUF);  // QREG only: (rank, start) of the last <= 32 admissions
-    // QREG only: the per-lane latency sums and makespans live in shared memory (touched once per 32
-    // admissions), not in three registers across the hot loop
-    long long* tel_s = reinterpret_cast<long long*>(dyn_smem + OFF_TEL);
-    int* mk_s = reinterpret_cast<int*>(dyn_smem + OFF_MK);
     // QREG: the shared-memory window address of dyn_smem, held in ONE register (opaque to the compiler,
     // which otherwise re-derives it from SR_CgaCtaId inside the hot loop)
     uint32_t sm32 = 0;
@@ -563,9 +557,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 
             // arrival window: lane l holds request wb + l
             int wb = 0, aw, sw = 0, ow = 0, rw;
-            // QREG (96 registers, none to spare): the rarely taken paths (window refill every 32 arrivals,
-            // output flush every 32 admissions) re-derive their pointers from (policy index, base)
-            // behind an opaque copy, so that no 64-bit pointer stays live across the hot loop
+            // QREG (96 registers, none to spare): the rarely taken path (window refill every 32 arrivals)
+            // re-derives its pointers from (policy index, base) behind an opaque copy, so that no 64-bit
+            // pointer stays live across the hot loop
             auto load_window = [&]() {
                 const int idx = wb + lane;
                 const bool in = idx < n;
@@ -585,14 +579,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                 Rec x; x.r = r; x.s = __shfl_sync(FULL, sw, l); x.o = __shfl_sync(FULL, ow, l);
                 x.a = __shfl_sync(FULL, aw, l); x.id = wb + l; return x;
             };
-            // output buffer: admission number m sits in lane m % 32 of warp 0 until 32 are there
-            // (QREG: b_id holds the RANK; id and arrival are looked up when the buffer is written)
-            // (QREG: (rank, start) go to a 32-entry buffer in shared memory; id, arrival and o are looked
-            // up when the buffer is written)
+            // non-QREG output buffer: admission number m sits in lane m % 32 of warp 0 until 32 are there
+            // (QREG: the start time waits at the request's rank in shared memory until the instance ends)
             int b_id = 0, b_t = 0, b_f = 0, b_lat = 0;
             auto flush = [&](int count) {
-                if (QREG) {
-                } else if (wrp == 0 && lane < count) {
+                if (!QREG && wrp == 0 && lane < count) {
                     const int id = b_id, lat = b_lat;
                     if (want_start) out_start[id] = b_t;
                     if (want_finish) out_finish[id] = b_f;
