@@ -45,9 +45,10 @@ L2_FLUSH_BYTES = 512 << 20
 # kernel's counting variant on the same inputs.  Peak = the SM issue rate, from the guide's unit
 # counts: SMs x 4 schedulers x 32 lanes x 1 warp-instruction/cycle x max SM clock.
 OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
-# HBM bytes per request and policy the same kernel must move: a, s, o (12) + rank (4) + order (4) +
-# start, finish (8) + latency for the p99 selection (4 written, 4 read back)
-SIM_BYTES_PER_REQUEST = 36
+# HBM bytes per request and policy the same kernel must move: a, s, o (12) + rank (4) +
+# start, finish (8) + latency for the p99 selection (4 written, 4 read back); the register-queue
+# kernels write their outputs in index order and never read order[]
+SIM_BYTES_PER_REQUEST = 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload come from the
 # committed `ncu --set full` summary of the same command (never from a run under the profiler here)
 SIM_PROFILE = os.path.join("profiles", "r02_kslots_full.md")
