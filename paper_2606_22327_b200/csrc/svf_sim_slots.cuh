@@ -188,11 +188,16 @@ __device__ __forceinline__ void reduce_add_max_min(uint32_t& a, int& b, int& c, 
         parity ^= 1;
         if (lane == 0) { sc[wrp][0] = (int)a; sc[wrp][1] = b; sc[wrp][2] = c; }
         __syncthreads();
-        const bool in = lane < WARPS;
-        const int l = in ? lane : 0;
-        a = __reduce_add_sync(FULL, in ? (uint32_t)sc[l][0] : 0u);
-        b = __reduce_max_sync(FULL, in ? sc[l][1] : INT_MIN);
-        c = __reduce_min_sync(FULL, in ? sc[l][2] : INT_MAX);
+        // every thread combines the warps' triples itself (broadcast loads, a few ALU operations): a second
+        // round of warp reductions costs their latency once more on the serial chain
+        uint32_t sa = 0; int sb = INT_MIN, scn = INT_MAX;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) {
+            sa += (uint32_t)sc[w][0];
+            sb = sc[w][1] > sb ? sc[w][1] : sb;
+            scn = sc[w][2] < scn ? sc[w][2] : scn;
+        }
+        a = sa; b = sb; c = scn;
     }
 }
 
