@@ -281,14 +281,6 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
 #define SVF_PUT2(ik, OP, k0)  if ((ik) & 1) { OP(k0 + 1) } else { OP(k0) }
 #define SVF_PUT4(ik, OP, k0)  if ((ik) & 2) { SVF_PUT2(ik, OP, k0 + 2) } else { SVF_PUT2(ik, OP, k0) }
 #define SVF_PUT8(ik, OP, k0)  if ((ik) & 4) { SVF_PUT4(ik, OP, k0 + 4) } else { SVF_PUT4(ik, OP, k0) }
-#ifndef SVF_PUT_SWITCH
-#define SVF_PUT_SWITCH 0
-#endif
-#if SVF_PUT_SWITCH
-#define SVF_PUT16(ik, OP)     switch (ik) { case 0: OP(0) break; case 1: OP(1) break; case 2: OP(2) break; case 3: OP(3) break; \
-    case 4: OP(4) break; case 5: OP(5) break; case 6: OP(6) break; case 7: OP(7) break; case 8: OP(8) break; case 9: OP(9) break; \
-    case 10: OP(10) break; case 11: OP(11) break; case 12: OP(12) break; case 13: OP(13) break; case 14: OP(14) break; default: OP(15) break; }
-#else
 // (two levels of uniform branches, then the four slots of the group under predicates: a quarter of the
 // code of the full tree)
 #define SVF_PUTG(ik, k0)  { const int j_ = (ik) & 3;                                          \
@@ -298,7 +290,6 @@ __device__ __forceinline__ uint32_t group_select_kth(const uint32_t* v, int n, i
     if (mine && j_ == 3) { f[k0 + 3] = fh; B[k0 + 3] = Bh; c[k0 + 3] = add; } }
 #define SVF_PUT16G(ik)        if ((ik) & 8) { if ((ik) & 4) SVF_PUTG(ik, 12) else SVF_PUTG(ik, 8) } else { if ((ik) & 4) SVF_PUTG(ik, 4) else SVF_PUTG(ik, 0) }
 #define SVF_PUT16(ik, OP)     if ((ik) & 8) { SVF_PUT8(ik, OP, 8) } else { SVF_PUT8(ik, OP, 0) }
-#endif
 #define SVF_PUT32(ik, OP)     if ((ik) & 16) { if ((ik) & 8) { SVF_PUT8(ik, OP, 24) } else { SVF_PUT8(ik, OP, 16) } } else { SVF_PUT16(ik, OP) }
 #define SVF_PUT32G(ik)        if ((ik) & 16) { if ((ik) & 8) { if ((ik) & 4) SVF_PUTG(ik, 28) else SVF_PUTG(ik, 24) } else { if ((ik) & 4) SVF_PUTG(ik, 20) else SVF_PUTG(ik, 16) } } else { SVF_PUT16G(ik) }
 // LAT (kernels that run as a few lone groups: latency matters, not the instruction count): the compact form
