@@ -374,6 +374,12 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
     // for instruction count; every other form runs as a few groups per SM and is tuned for the length of its
     // serial chain (measured: the choices below are worth 1-2 % each there and cost the bench kernel 0.5-3 %)
     constexpr bool LAT = !(QREG && QW == 1);
+    // one bitmap word per lane (the bench shape): the bitmap is INTERLEAVED over the lanes, rank r = bit r >> 5
+    // of lane r & 31, and the lowest waiting rank is ONE warp reduction (every lane offers its lowest set bit
+    // as (bit << 5) | lane = the rank itself): no ballot + shuffle, no cached word of the head (5.53 -> 5.37 ms
+    // per bench step).  With more words per lane the lanes hold consecutive ranks and the head's word is
+    // cached (measured: the interleaved form costs configs[4] 10-20 % there)
+    constexpr bool ILV = QREG && QW == 1;
     constexpr int RB = REC4 ? 4 : 8;                             // bytes of a waiting record in shared memory
     constexpr int OFF_BITS = QRANKS * RB;
     static_assert(K == 16 || (K == 32 && THREADS == 32 && (!QREG || REC4)), "the slot macros are written out for 16 slots per thread (32: one-warp groups)");
@@ -528,6 +534,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             for (int w = 0; w < QW; ++w) qword[w] = 0;
             // lowest waiting rank (INT_MAX if none), the rest of its word above it, the word's first rank
             auto queue_head = [&](uint32_t& rest, int& wbase_, uint32_t& bit_) -> int {
+                if constexpr (ILV) {        // (an empty lane offers (0 - 1) << 5 | lane, above every rank as unsigned)
+                    const uint32_t key = __reduce_min_sync(FULL, ((uint32_t)(__ffs(qword[0]) - 1) << 5) | (uint32_t)lane);
+                    return (int)key < 0 ? INT_MAX : (int)key;
+                }
 #pragma unroll
                 for (int w = 0; w < QW; ++w) {
                     const uint32_t nz = __ballot_sync(FULL, qword[w] != 0u);
@@ -622,7 +632,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                 asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u), "r"(qword[w]) : "memory");
                             __syncwarp();
                         }
-                        if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(rw >> 5) * 4u), "r"(1u << (rw & 31)) : "memory");
+                        if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(ILV ? (rw & 31) : (rw >> 5)) * 4u), "r"(1u << (ILV ? (rw >> 5) : (rw & 31))) : "memory");
                     } else {
                         // nobody may still be reading the bitmap for the previous step
                         if (!arrived) G::sync();
@@ -773,7 +783,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                             peak = p2 > peak ? p2 : peak;
                         }
                         if (QREG) {
-                            if constexpr (QW <= 2) {
+                            if constexpr (ILV) {
+                                if (lane == (head.r & 31)) qword[0] &= ~(1u << (head.r >> 5));
+                            } else if constexpr (QW <= 2) {
 #pragma unroll
                                 for (int w = 0; w < QW; ++w)      // the head's bit (a uniform one-hot word) leaves its lane's word
                                     if (w * 32 + lane == (hbase >> 5)) qword[w] ^= hbit;
@@ -797,7 +809,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                             // of it, `hrest`), else the lowest set bit of the later words; its (s, o) come
                             // from shared memory
                             int r;
-                            if (hrest) {
+                            if (!ILV && hrest) {
                                 hbit = hrest & (0u - hrest);
                                 hrest ^= hbit;
                                 r = hbase + (31 - __clz(hbit));
