@@ -45,7 +45,9 @@
 // WAITING QUEUE: bitmap over ranks (keys are time-invariant, so the presort fixes the order).
 //  * QREG (one warp per instance, at most 8,192 requests): QW 32-bit words per lane in registers
 //    (QW = 1, 2 or 8: 1,024 ranks per word index), mirrored in shared memory where arrivals set their
-//    bits with one atomic OR each; the (s, o) of every request sits in shared memory by rank, staged
+//    bits with one atomic OR each; with one word per lane (the bench shape) the ranks are interleaved
+//    over the lanes and the head is one warp reduction, with more words a lane holds consecutive ranks
+//    and the head's word is cached uniformly (ILV in the kernel); the (s, o) of every request sits in shared memory by rank, staged
 //    once per instance, so picking the next head never waits for global memory; id and arrival are
 //    only looked up when the outputs are written.  Up to 2,048 requests the records are 8 bytes; above
 //    (REC4) they are PACKED into one word, s in the low bits, the split taken from the widths of the
