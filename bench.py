@@ -294,7 +294,7 @@ def run_ours(args):
         step(profile=phase)
     B.set_profiling(False)
     phase = np.array(phase, dtype=np.float64)            # [calls, 4]
-    sim_ms = float(phase[:, 1].mean())                   # the one k_sim_slots launch of a step (all four policies)
+    sim_ms = float(np.median(phase[:, 1]))               # the one k_sim_slots launch of a step (all four policies); median: one slow launch must not move it
     share = {"phase_a_keys_sort_rank": float(phase[:, 0].sum() / phase[:, 3].sum()),
              "phase_b_simulator": float(phase[:, 1].sum() / phase[:, 3].sum()),
              "phase_c_p99": float(phase[:, 2].sum() / phase[:, 3].sum())}
