@@ -620,6 +620,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
             while (started < n) {
                 // 2. ARRIVE (1. COMPLETE is implicit: a slot is dead once f <= t)
                 bool arrived = false;
+                int rmin = INT_MAX;                  // ILV: lowest rank among this step's arrivals
                 while (next < n) {
                     if (next >= wb + 32) { wb = next; load_window(); }
                     const int idx = wb + lane;
@@ -634,6 +635,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                 asm volatile("st.shared.u32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u), "r"(qword[w]) : "memory");
                             __syncwarp();
                         }
+                        if (ILV) { const int rm = __reduce_min_sync(FULL, v ? rw : INT_MAX); rmin = rm < rmin ? rm : rmin; }
                         if (v) asm volatile("red.shared.or.b32 [%0], %1;" :: "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(ILV ? (rw & 31) : (rw >> 5)) * 4u), "r"(1u << (ILV ? (rw >> 5) : (rw & 31))) : "memory");
                     } else {
                         // nobody may still be reading the bitmap for the previous step
@@ -671,7 +673,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
 #pragma unroll
                         for (int w = 0; w < QW; ++w)
                             asm volatile("ld.shared.u32 %0, [%1];" : "=r"(qword[w]) : "r"(sm32 + (uint32_t)OFF_BITS + (uint32_t)(w * 32 + lane) * 4u) : "memory");
-                        const int r0 = queue_head(hrest, hbase, hbit);      // (arrivals set bits: the queue is not empty)
+                        // (ILV: the head after the arrivals is the lower of the old head and the lowest arriving rank:
+                        // known before the bitmap has made its round trip through shared memory)
+                        const int r0 = ILV ? (rmin < head.r ? rmin : head.r) : queue_head(hrest, hbase, hbit);      // (arrivals set bits: the queue is not empty)
                         if (r0 != head.r) {
                             const int2 v = lds_rec(r0);
                             head.r = r0; head.s = v.x; head.o = v.y;
