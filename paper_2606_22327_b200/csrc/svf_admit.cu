@@ -82,11 +82,12 @@ __device__ __forceinline__ int64_t block_incl_scan_i64(int64_t v, int64_t* warp_
 }
 
 // ---- the maximal feasible prefix by bisection (a4 + a5), one CTA -------------------------------
-constexpr int AP_THREADS = 1024;
+constexpr int AP_THREADS = 1024;                     // the wide form: up to 8,192 entries on chip
 constexpr int AP_IPT = 8;
 constexpr int AP_CAP = AP_THREADS * AP_IPT;          // running + candidate entries held on chip
 constexpr int AP_RUN_MAX = AP_CAP / 2;               // larger running sets take the serial path
-constexpr size_t AP_SMEM = (size_t)2 * AP_CAP * 8 + (size_t)AP_CAP * 4 + (size_t)(AP_THREADS / 32) * SORT_RADIX * 4;
+constexpr size_t ap_smem_bytes(int threads) { return (size_t)2 * threads * AP_IPT * 8 + (size_t)threads * AP_IPT * 4 + (size_t)(threads / 32) * SORT_RADIX * 4; }
+constexpr size_t AP_SMEM = ap_smem_bytes(AP_THREADS);
 
 // fast[0] = 1: this kernel has answered (outputs written); 0: the serial kernels must run, and
 // rsorted_out holds the running set in their order (latest finish first, ties in input order).
@@ -99,7 +100,7 @@ struct AdmitFused {
     uint64_t* sorted_words_out;              // or NULL
 };
 
-template <bool FUSED>
+template <bool FUSED, int AP_THREADS>
 __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64_t n_wait, const int32_t* __restrict__ w_s,
                                                                 const int32_t* __restrict__ w_o, int n_run,
                                                                 const int32_t* __restrict__ r_kv,
@@ -112,6 +113,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
                                                                 int32_t* __restrict__ status_out, AdmitFused fu)
 {
     constexpr int WARPS = AP_THREADS / 32;
+    constexpr int AP_CAP = AP_THREADS * AP_IPT;          // running + candidate entries held on chip
     extern __shared__ __align__(16) char ap_smem[];
     uint64_t* buf0 = reinterpret_cast<uint64_t*>(ap_smem);
     uint64_t* buf1 = buf0 + AP_CAP;
@@ -277,7 +279,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         }
         if (lane == 31) { wsum_s[wrp] = si; wcnt_s[wrp] = ci; }
         __syncthreads();
-        int64_t ws = wsum_s[lane]; int wc = wcnt_s[lane];       // WARPS == 32: one warp total per lane
+        int64_t ws = lane < WARPS ? wsum_s[lane] : 0; int wc = lane < WARPS ? wcnt_s[lane] : 0;       // one warp total per lane
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const int64_t x = __shfl_up_sync(FULL, ws, d); const int y = __shfl_up_sync(FULL, wc, d);
@@ -291,7 +293,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
             if (rk[i] < m) { pre += kv[i]; ++cnt; bad |= pre + (int64_t)rem[i] * cnt > M; }
         return __syncthreads_or(bad) == 0;               // also fences wsum_s / wcnt_s for the next call
     };
-    static_assert(WARPS == 32, "the second scan level holds one warp total per lane");
+    static_assert(WARPS <= 32, "the second scan level holds one warp total per lane");
     // the same probe in 32 bits when the numbers allow it (M < 2^26 and rem * count < 2^30: every config
     // of the paper's shape): sums SATURATE at 2^26 > M (all terms are >= 0, so a saturated sum is a
     // violated one and saturating addition stays associative), one shuffle per scan step instead of
@@ -343,7 +345,7 @@ __global__ void __launch_bounds__(AP_THREADS, 1) k_admit_prefix(int64_t M, int64
         for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(FULL, ci, d); if (lane >= d) ci += y; }
         if (lane == 31) wcnt_s[wrp] = ci;
         __syncthreads();
-        int wc = wcnt_s[lane];
+        int wc = lane < WARPS ? wcnt_s[lane] : 0;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(FULL, wc, d); if (lane >= d) wc += y; }
         int q = ci - c + (wrp > 0 ? __shfl_sync(FULL, wc, wrp - 1) : 0);
@@ -625,11 +627,22 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     if (n_wait + n_run <= AP_CAP) {
         // a queue and a running set that fit one CTA's shared memory: the whole decision in ONE launch
         AdmitFused fu{policy, O0, O1, w_a, w_bit, sorted_words_out};
-        if (cudaFuncSetAttribute(k_admit_prefix<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
-        admit_mark(1, st);
-        admit_mark(2, st);
-        k_admit_prefix<true><<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, nullptr, nullptr, nullptr,
-                                                             nullptr, n_admitted_out, admitted_idx_out, status_out, fu);
+        // the narrowest CTA that holds the entries: every barrier and block scan of the sorts and of the
+        // 14 bisection probes costs by the warps taking part (kernel 29 -> 17 ... 23 us for a serving queue)
+#define SVF_AP_LAUNCH(T)                                                                                        \
+        do {                                                                                                    \
+            if (cudaFuncSetAttribute(k_admit_prefix<true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,      \
+                                     (int)ap_smem_bytes(T)) != cudaSuccess) return SVF_ECUDA;                   \
+            admit_mark(1, st);                                                                                  \
+            admit_mark(2, st);                                                                                  \
+            k_admit_prefix<true, T><<<1, T, ap_smem_bytes(T), st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, nullptr, nullptr, \
+                                                                    nullptr, nullptr, n_admitted_out, admitted_idx_out, status_out, fu); \
+        } while (0)
+        const int64_t entries = n_wait + n_run;
+        if (entries <= 256 * AP_IPT) SVF_AP_LAUNCH(256);
+        else if (entries <= 512 * AP_IPT) SVF_AP_LAUNCH(512);
+        else SVF_AP_LAUNCH(AP_THREADS);
+#undef SVF_AP_LAUNCH
         ++g_launches_admit;
         admit_mark(3, st);
         return cudaGetLastError() == cudaSuccess ? SVF_OK : SVF_ECUDA;
@@ -656,8 +669,8 @@ extern "C" int svf_admit(int policy, int64_t M, int32_t t, int64_t n_wait, const
     const bool prefix = n_run <= AP_RUN_MAX;
     if (prefix) admit_mark(2, st);            // (else the running set's device-wide sort still belongs to phase 1)
     if (prefix) {
-        if (cudaFuncSetAttribute(k_admit_prefix<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
-        k_admit_prefix<false><<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
+        if (cudaFuncSetAttribute(k_admit_prefix<false, AP_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AP_SMEM) != cudaSuccess) return SVF_ECUDA;
+        k_admit_prefix<false, AP_THREADS><<<1, AP_THREADS, AP_SMEM, st>>>(M, n_wait, w_s, w_o, (int)n_run, r_kv, r_rem, w.wsort.plan, w.flags, w.r1,
                                                               w.fast, n_admitted_out, admitted_idx_out, status_out, AdmitFused{});
         ++g_launches_admit;
     } else {
