@@ -715,6 +715,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                         }
                         int eidx = INT_MAX;
                         if (use_ext) {
+                            int elive = REGCAP - 1;             // highest live ext slot of this thread
                             for (int q = REGCAP + tid; q < hw; q += THREADS) {
                                 const int e = q - REGCAP;
                                 const int fk = ef[e];
@@ -725,9 +726,15 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 32 && QREG) ? (QW == 1 ? 
                                     eB[e] += add + (uint32_t)fk;
                                     if (COUNT) cntU += 1;
                                 }
-                                if (x >> 31) eidx = eidx < q ? eidx : q;
+                                if (x >> 31) eidx = eidx < q ? eidx : q; else elive = q;
                                 if (COUNT) cntE += (long long)((x >> 31) ^ 1u);
                             }
+                            // the mark comes back down to the highest live ext slot: once the running set fits the
+                            // registers again, the passes stop walking dead ext slots in global memory (configs[3]
+                            // under 1-bit SVF peaks at 2,355 running requests for a sixth of its admissions)
+                            uint32_t z = 0; int emn = 0;
+                            reduce_add_max_min<THREADS>(z, elive, emn, red, rparity);
+                            hw = elive + 1;
                         }
                         acc += acc1;
                         reduce_add_max_min<THREADS>(acc, viol, fkey, red, rparity);
