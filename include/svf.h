@@ -133,6 +133,35 @@ int svf_admit(int policy, int64_t M, int32_t t,
               int64_t* n_admitted_out, int32_t* admitted_idx_out, uint64_t* sorted_words_out,
               int32_t* status_out, void* ws, size_t ws_bytes, void* stream);
 
+/* svf_admit for a caller that may not allocate device memory: same arguments, outputs, data errors
+ * and answer as svf_admit, minus `ws` / `ws_bytes`.  Meant for the place this decision is taken in
+ * production -- the step loop of a serving engine, or a plug-in inside one.  Such a process gives
+ * nearly all HBM to its KV-cache pool at start-up, so a later cudaMalloc may simply fail, and
+ * cudaMalloc / cudaFree synchronise the device and would stall the decode stream every step; other
+ * hosts forbid allocation outside their own pool, or offer no allocator to a plain C caller.
+ * Here the scratch is a fixed array inside the library image (SVF_ADMIT_STATIC_BYTES of device
+ * memory on EVERY GPU that loads the library, held until the process exits).  The call issues no
+ * cudaMalloc / cudaFree and calls no allocating routine; inputs and outputs remain the caller's.
+ *  - Limit: n_wait <= SVF_ADMIT_STATIC_MAX_WAIT and n_run <= SVF_ADMIT_STATIC_MAX_RUN; anything
+ *    larger returns SVF_EWORKSPACE (take svf_admit with your own buffer), before the device is
+ *    touched.  With svf_set_profiling switched on it returns SVF_EINVAL (that aid creates events).
+ *  - First call on each device: it looks up the array's device address (the device that is current
+ *    at the call), which may load the library's device code there.  Make that first call during
+ *    start-up, ahead of any stream capture; later calls only enqueue kernels and memsets.
+ *  - All calls on one GPU share the one array and it still holds whatever the previous call left;
+ *    everything the kernels need zeroed is cleared on `stream` at the start of each call.  Two
+ *    calls that can overlap on the same GPU (different streams, or different host threads) RACE:
+ *    order them on one stream or with events.  svf_admit with separate buffers has no such limit. */
+#define SVF_ADMIT_STATIC_MAX_WAIT 65536
+#define SVF_ADMIT_STATIC_MAX_RUN  8192
+#define SVF_ADMIT_STATIC_BYTES    (3 << 20)
+int svf_admit_static(int policy, int64_t M, int32_t t,
+                     int64_t n_wait, const int32_t* w_s, const int32_t* w_o, const int32_t* w_a,
+                     const uint8_t* w_bit, int32_t O0, int32_t O1,
+                     int64_t n_run, const int32_t* r_kv, const int32_t* r_rem,
+                     int64_t* n_admitted_out, int32_t* admitted_idx_out, uint64_t* sorted_words_out,
+                     int32_t* status_out, void* stream);
+
 /* a1-a7: the batched discrete-time simulator (P:L87-104 model; Alg. 1 Process 2).
  * Per instance, from t = a_0:  COMPLETE (k_i + o_i == t) -> ARRIVE (a_i <= t) -> ADMIT (pop
  * the head of the (key, arrival, id) order while the forward-looking check passes; stop at the

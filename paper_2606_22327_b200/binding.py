@@ -21,7 +21,7 @@ POLICY_NAMES = {SVF: "svf", SVF_1BIT: "svf_1bit", SJF: "sjf", FCFS: "fcfs"}
 OK, EINVAL, EWORKSPACE, ECUDA = 0, 1, 2, 3
 ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
-EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_simulate_workspace_bytes",
+EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_admit_static", "svf_simulate_workspace_bytes",
            "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies",
            "svf_volume_lower_bound_workspace_bytes", "svf_volume_lower_bound", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
            "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
@@ -68,6 +68,11 @@ def lib():
                                 C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p,
                                 C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                 C.c_void_p, C.c_size_t, C.c_void_p]
+        L.svf_admit_static.restype = C.c_int
+        L.svf_admit_static.argtypes = [C.c_int, C.c_int64, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int64,
+                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p]
         L.svf_simulate_workspace_bytes.restype = C.c_size_t
         L.svf_simulate_workspace_bytes.argtypes = [C.POINTER(_Trace)]
         L.svf_simulate.restype = C.c_int
@@ -249,6 +254,30 @@ def svf_admit(policy, M, t, w_s, w_o, w_a, w_bit, O0, O1, r_kv, r_rem, want_sort
     _check(rc, "svf_admit")
     _hold(ws, stream)
     out._ws = ws  # keep the scratch alive until the caller drops the result
+    return out
+
+
+ADMIT_STATIC_MAX_WAIT, ADMIT_STATIC_MAX_RUN = 65536, 8192     # the limits include/svf.h states
+
+
+def svf_admit_static(policy, M, t, w_s, w_o, w_a, w_bit, O0, O1, r_kv, r_rem, out: AdmitOut,
+                     stream=None) -> AdmitOut:
+    """svf_admit for a caller that must not allocate device memory (a scheduler inside a serving
+    engine whose KV-cache pool already owns the HBM, where cudaMalloc can fail and would stall the
+    decode stream).  The scratch is a fixed array inside the library, so this binding allocates
+    nothing either: `out` (an AdmitOut you made once at start-up; sorted_words may be None) is
+    required and is filled in place.  Raises SvfError(EWORKSPACE) above 65,536 waiting or 8,192
+    running requests.  Calls share the one array per GPU: keep them on one stream, or order them."""
+    nw, nr = int(w_s.numel()), int(r_kv.numel())
+    rc = lib().svf_admit_static(int(policy), int(M), int(t), nw, _ptr(w_s, torch.int32, "w_s"),
+                                _ptr(w_o, torch.int32, "w_o"), _ptr(w_a, torch.int32, "w_a"),
+                                _ptr(w_bit, torch.uint8, "w_bit"), int(O0), int(O1), nr,
+                                _ptr(r_kv, torch.int32, "r_kv"), _ptr(r_rem, torch.int32, "r_rem"),
+                                _ptr(out.n_admitted, torch.int64, "n_admitted"),
+                                _ptr(out.admitted_idx, torch.int32, "admitted_idx"),
+                                _ptr(out.sorted_words, torch.int64, "sorted_words"),
+                                _ptr(out.status, torch.int32, "status"), _stream(stream))
+    _check(rc, "svf_admit_static")
     return out
 
 

@@ -16,7 +16,8 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 LIB = os.path.join(CSRC, "libsvf_b200.so")
 INCLUDE = os.path.join(os.path.dirname(_DIR), "include")
-SOURCES = ["svf_api.cu", "svf_keys.cu", "svf_sort.cu", "svf_admit.cu", "svf_simulate.cu"]
+SOURCES = ["svf_api.cu", "svf_keys.cu", "svf_sort.cu", "svf_admit.cu", "svf_simulate.cu",
+           "svf_admit_static.cu"]
 HEADERS = ["svf_internal.cuh", "svf_state.cuh", "svf_sim_slots.cuh", "svf_segsort.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]

@@ -221,3 +221,32 @@ def test_compute_calls_return_ecuda_without_a_device(svf_lib):
                          capture_output=True, text=True, timeout=300)
     assert out.returncode == 0, out.stderr
     assert out.stdout.strip() == ",".join(["3"] * 7), out.stdout
+
+
+def test_static_admit_checks_arguments_and_its_size_limit_on_the_host(svf_lib):
+    """svf_admit_static (scratch inside the library, for callers that may not allocate): argument
+    errors and the stated maximum are found before the device is touched; the maximum fits the array."""
+    L = svf_lib
+    f = L.svf_admit_static
+    f.restype = C.c_int
+    f.argtypes = [C.c_int, C.c_int64, C.c_int32, C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 7
+    k = C.c_int64(0)
+    kp = C.addressof(k)
+    args = lambda policy, n_wait, n_run, out=kp: (policy, 100, 0, n_wait, None, None, None, None, 1, 1, n_run, None, None, out, None, None, None, None)
+    assert f(*args(9, 0, 0)) == 1                      # unknown policy
+    assert f(*args(0, -1, 0)) == 1                     # negative size
+    assert f(*args(0, 0, 0, None)) == 1                # nowhere to write the answer
+    assert f(*args(0, 5, 0)) == 1                      # null arrays
+    buf = (C.c_int32 * 70000)()
+    p = C.addressof(buf)
+    wide = lambda n_wait, n_run: (0, 100, 0, n_wait, p, p, p, None, 1, 1, n_run, p, p, kp, None, None, None, None)
+    assert f(*wide(65537, 0)) == 2                     # beyond SVF_ADMIT_STATIC_MAX_WAIT
+    assert f(*wide(10, 8193)) == 2                     # beyond SVF_ADMIT_STATIC_MAX_RUN
+    hdr = open(os.path.join(ROOT, "include", "svf.h")).read()
+    mw = int(re.search(r"SVF_ADMIT_STATIC_MAX_WAIT\s+(\d+)", hdr).group(1))
+    mr = int(re.search(r"SVF_ADMIT_STATIC_MAX_RUN\s+(\d+)", hdr).group(1))
+    sh = int(re.search(r"SVF_ADMIT_STATIC_BYTES\s+\((\d+) << 20\)", hdr).group(1))
+    L.svf_admit_workspace_bytes.restype = C.c_size_t
+    L.svf_admit_workspace_bytes.argtypes = [C.c_int64, C.c_int64]
+    assert (mw, mr) == (65536, 8192)
+    assert L.svf_admit_workspace_bytes(mw, mr) <= sh << 20
