@@ -51,25 +51,19 @@ OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
 SIM_BYTES_PER_REQUEST = 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload come from the
 # committed `ncu --set full` summary of the same command (never from a run under the profiler here)
-SIM_PROFILE = os.path.join("profiles", "r02_kslots_full.md")
+SIM_PROFILE = os.path.join("profiles", "r02_kslots_traffic.json")
 
 
 def profiled_dram_traffic():
-    """(bytes per k_sim_slots launch, source) read from the committed ncu summary, or (None, why)."""
+    """(bytes per k_sim_slots launch, source) from the small JSON that sits beside the committed
+    `ncu --set full` summary and names the table it was taken from, or (None, why)."""
     path = os.path.join(ROOT, SIM_PROFILE)
     try:
-        rd = wr = None
-        for line in open(path):
-            f = [x.strip() for x in line.split("|")]
-            if len(f) >= 4 and f[1] == "dram__bytes_read.sum":
-                rd = float(f[3]) * {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0}[f[2]]
-            if len(f) >= 4 and f[1] == "dram__bytes_write.sum":
-                wr = float(f[3]) * {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0}[f[2]]
-        if rd is not None and wr is not None:
-            return rd + wr, f"{SIM_PROFILE} (dram__bytes_read.sum + dram__bytes_write.sum of one launch)"
-    except OSError:
-        pass
-    return None, f"{SIM_PROFILE} not found"
+        rec = json.load(open(path))
+        total = float(rec["dram__bytes_read.sum"]) + float(rec["dram__bytes_write.sum"])
+        return total, f"{SIM_PROFILE}: {rec.get('table', '?')} (kernel source as of commit {rec.get('commit', '?')})"
+    except (OSError, KeyError, ValueError):
+        return None, f"{SIM_PROFILE} missing or unreadable"
 
 
 def parse_args():
@@ -83,6 +77,7 @@ def parse_args():
     ap.add_argument("--lam", type=float, default=4.0)
     ap.add_argument("--e2e-chunks", type=int, default=8, help="instance chunks (streams) of the end-to-end leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel and per-config extras")
+    ap.add_argument("--extras-file", default=None, help=f"where the extras go (default {EXTRAS_FILE}); never stdout")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-oracle-extras", action="store_true", help="extras without the oracle timed beside each config")
     return ap.parse_args()
@@ -218,6 +213,55 @@ def workload_config(args, n_inst=None):
             "instances_per_gpu": n_inst or args.instances, "requests_per_instance": args.requests,
             "M": 300000, "policies": list(POLICY_NAMES),
             "cache": f"L2 flushed between timed steps (write of {L2_FLUSH_BYTES >> 20} MiB)"}
+
+
+# ---------------------------------------------------------------------------------------------
+# the ONE line the driver reads: compact (<= HEADLINE_MAX_BYTES), strict JSON, printed before any
+# extra is run; everything else goes to EXTRAS_FILE
+# ---------------------------------------------------------------------------------------------
+HEADLINE_MAX_BYTES = 4096
+EXTRAS_FILE = os.path.join("gpurun_out", "bench_extras.json")
+HEADLINE_KEYS = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                 "scaling", "vs_baseline", "dtype", "data", "config", "decisions_per_sec", "clocks", "e2e",
+                 "gpu_launches", "roofline", "cpu_baseline")
+ROOFLINE_KEYS = ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic", "kernel_ms", "share_of_step",
+                 "algorithmic_ops_per_launch", "hbm_frac")
+
+
+def _sig(x, digits=7):
+    """floats to `digits` significant figures (the line is read by a program, then by people)"""
+    if isinstance(x, float):
+        return float(f"{x:.{digits}g}") if x == x and abs(x) != float("inf") else None
+    if isinstance(x, dict):
+        return {k: _sig(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_sig(v, digits) for v in x]
+    return x
+
+
+def build_headline(full: dict, extras_file=None) -> str:
+    """The compact headline of `full` (run_ours's whole record) as one line of strict JSON of at most
+    HEADLINE_MAX_BYTES: the contract's keys, the scalar fields of `roofline`, `cpu_baseline`, `e2e`.
+    Raises if a required key is missing or the line is too long (a test builds it from canned numbers)."""
+    head = {k: full[k] for k in HEADLINE_KEYS if k in full}
+    missing = [k for k in HEADLINE_KEYS if k not in head and k != "cpu_baseline"]
+    if missing:
+        raise KeyError(f"bench headline lacks {missing}")
+    roof = full["roofline"]
+    head["roofline"] = {k: roof.get(k) for k in ROOFLINE_KEYS}
+    if isinstance(roof.get("share_of_step"), dict):      # the dominant kernel's share only
+        head["roofline"]["share_of_step"] = roof["share_of_step"].get("phase_b_simulator")
+    if isinstance(roof.get("hbm"), dict):
+        head["roofline"]["hbm_frac"] = roof["hbm"].get("frac")
+    for k in ("fingerprint_fnv1a64",):
+        if k in full:
+            head[k] = full[k]
+    if extras_file:
+        head["extras_file"] = extras_file
+    text = json.dumps(_sig(_finite(head)), allow_nan=False, separators=(",", ":"))
+    if len(text.encode()) > HEADLINE_MAX_BYTES:
+        raise ValueError(f"bench headline is {len(text.encode())} bytes (> {HEADLINE_MAX_BYTES})")
+    return text
 
 
 # ---------------------------------------------------------------------------------------------
@@ -431,23 +475,44 @@ def run_ours(args):
     }
     peak = hbm_peak
     line["fingerprint_fnv1a64"] = T.trace_fingerprint(batch)
-    if not args.no_extras:
-        line["kernels"] = kernel_extras(B, torch, dev, peak)
-        line["admit_sweep"] = admit_sweep(B, torch, dev, peak)
-        line["configs"] = config_extras(B, torch, dev, args, with_oracle=not (args.no_oracle_extras or args.no_cpu_baseline))
-        line["ratio_to_lower_bound"] = bound_extras(B, torch, dev, args)
-        line["stochastic_regime"] = stochastic_extras(B, torch, dev)
-        # the paper's own metrics on the bench batch, per policy, this rank
-        from paper_2606_22327_b200 import report as RP
-        line["paper_metrics"] = {
-            name: RP.paper_metrics(dt_dev.arrival, dt_dev.output, o.finish[: batch.n_requests], dt_dev.offsets, o.status)
-            for name, o in zip(POLICY_NAMES, outs)}
-        line["paper_metrics"]["units"] = "per-token latency in model steps per output token; throughput in tokens per step per instance"
+    # the reported CPU baseline first (oracle on the host cores), then the headline, THEN the extras:
+    # nothing an extra does (an exception, a crash, a long line) can cost the line the driver reads
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args)
-    print(json.dumps(_finite(line)), flush=True)
+    extras_path = None if args.no_extras else (args.extras_file or EXTRAS_FILE)
+    print(build_headline(line, extras_path), flush=True)
+    if extras_path is not None:
+        extras = dict(_finite(line))
+        legs = (("kernels", lambda: kernel_extras(B, torch, dev, peak)),
+                ("admit_sweep", lambda: admit_sweep(B, torch, dev, peak)),
+                ("configs", lambda: config_extras(B, torch, dev, args, with_oracle=not (args.no_oracle_extras or args.no_cpu_baseline))),
+                ("ratio_to_lower_bound", lambda: bound_extras(B, torch, dev, args)),
+                ("stochastic_regime", lambda: stochastic_extras(B, torch, dev)),
+                ("paper_metrics", lambda: paper_metrics_extras(B, dt_dev, outs, batch)))
+        for name, leg in legs:
+            try:
+                extras[name] = _finite(leg())
+            except Exception as e:   # recorded, never fatal: the headline is already out
+                extras[name] = {"error": f"{type(e).__name__}: {e}"}
+            try:
+                full_path = extras_path if os.path.isabs(extras_path) else os.path.join(ROOT, extras_path)
+                os.makedirs(os.path.dirname(full_path), exist_ok=True)
+                with open(full_path + ".tmp", "w") as f:
+                    json.dump(extras, f, indent=1)
+                os.replace(full_path + ".tmp", full_path)
+            except OSError as e:
+                print(f"bench.py: could not write {extras_path}: {e}", file=sys.stderr)
     if world > 1:
         dist.destroy_process_group()
+
+
+def paper_metrics_extras(B, dt_dev, outs, batch):
+    """the paper's own metrics on the bench batch, per policy, this rank."""
+    from paper_2606_22327_b200 import report as RP
+    res = {name: RP.paper_metrics(dt_dev.arrival, dt_dev.output, o.finish[: batch.n_requests], dt_dev.offsets, o.status)
+           for name, o in zip(POLICY_NAMES, outs)}
+    res["units"] = "per-token latency in model steps per output token; throughput in tokens per step per instance"
+    return res
 
 
 def _finite(x):
@@ -531,8 +596,9 @@ def admit_sweep(B, torch, dev, peak):
                         "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": W / ms * 1e3,
                         "phase_ms": {"keys_and_validation": float(ph[0]), "sorts": float(ph[1]), "admission": float(ph[2]),
                                      "whole_call_under_events": float(ph[3])},
-                        "roofline": {"bound": "hbm", "achieved": algo / ms / 1e6, "peak": peak, "unit": "GB/s",
-                                     "frac": algo / ms / 1e6 / peak, "algorithmic_bytes": algo,
+                        # at these sizes the call is a short chain of small launches (or one CTA): latency, not
+                        # bandwidth, sets the time; the bytes are reported as a rate, without an HBM fraction
+                        "roofline": {"bound": "latency", "achieved": algo / ms / 1e6, "unit": "GB/s", "algorithmic_bytes": algo,
                                      "note": ("one launch, one CTA: validation, keys, both sorts and the bisection in shared memory (the phase "
                                               "split does not apply: all under 'admission'); bound by one SM's issue rate and barriers") if fused else
                                              "a chain of 13 small launches: launch latency, not bandwidth, sets the time at these sizes"}})

@@ -355,13 +355,26 @@ def _admit_both(B, oracle, policy, M, st, O0=179, O1=887):
 
 
 @pytest.mark.parametrize("n_wait,n_run", [(0, 0), (0, 50), (1, 0), (37, 0), (1024, 256), (5000, 1024),
-                                           (5001, 1024), (70_000, 4096), (1 << 18, 300), (3000, 6000)])
+                                           (5001, 1024), (70_000, 4096), (1 << 18, 300), (3000, 6000),
+                                           (2049, 0), (3000, 1000), (4096, 0)])     # 2049..4096 entries: the 512-thread one-launch form
 def test_admit_matches_oracle(B, oracle, n_wait, n_run):
     M = 1_000_000 if n_run <= 4096 else 6_000_000        # (3000, 6000): beyond the 4096 register slots
+    if n_wait + n_run in (2049, 4096):
+        M = 90_000                                       # tight: the bisection's answer lies inside the window
     st = _admit_state(n_wait + n_run, n_wait, n_run, M)
     ks = [_admit_both(B, oracle, policy, M, st) for policy in range(4)]
     if n_wait >= 1024 and n_run <= 1024:
         assert max(ks) > 0
+
+
+def test_admit_512_thread_form_with_tied_remaining_steps(B, oracle):
+    """2049..4096 entries take k_admit_prefix<true, 512> (its second scan level and shared-memory opt-in);
+    here with a running set whose remaining steps are heavily tied (10 distinct values)."""
+    w_s, w_o, w_a, w_bit, r_kv, r_rem = _admit_state(41, 2600, 900, 1_000_000)
+    r_rem = (r_rem % 10 + 1).astype(np.int32) * 100
+    for M in (700_000, 1_000_000, 1_400_000):
+        ks = [_admit_both(B, oracle, policy, M, (w_s, w_o, w_a, w_bit, r_kv, r_rem)) for policy in range(4)]
+    assert max(ks) > 0
 
 
 def test_admit_wide_budget_takes_the_sorted_array_kernel(B, oracle):

@@ -49,10 +49,10 @@ def _properties(out, tr):
     assert (out.peak_kv.cpu().numpy()[: tr.n_instances] <= tr.M).all()
 
 
-@pytest.mark.parametrize("lam", [2.0, 8.0])
+@pytest.mark.parametrize("lam", [2.0, 4.0, 8.0])
 def test_config3_full_size_other_rates(B, oracle, lam):
-    """configs[2]: 4,096 instances x 1,000 requests at Poisson rates 2 and 8 (rate 4 is the bench
-    launch, tested elsewhere), all four policies in the one-launch call, EVERY instance and field."""
+    """configs[2]: 4,096 instances x 1,000 requests at Poisson rates 2, 4 (the launch bench.py times)
+    and 8, all four policies in the one-launch call, EVERY instance and field."""
     import torch
     tr = T.config3(n_instances=4096, lam=lam)
     outs = B.svf_simulate_policies(B.DeviceTrace.from_host(tr), [0, 1, 2, 3])
