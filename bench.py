@@ -51,17 +51,28 @@ OPS_PER_EXAMINED, OPS_PER_UPDATED = 4, 2
 SIM_BYTES_PER_REQUEST = 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_sim_slots launch on this workload come from the
 # committed `ncu --set full` summary of the same command (never from a run under the profiler here)
-SIM_PROFILE = os.path.join("profiles", "r02_kslots_traffic.json")
+SIM_PROFILE = os.path.join("profiles", "r03_kslots_traffic.json")
+
+
+def _sources_sha256(files):
+    import hashlib
+    h = hashlib.sha256()
+    for f in files:
+        h.update(open(os.path.join(ROOT, f), "rb").read())
+    return h.hexdigest()
 
 
 def profiled_dram_traffic():
     """(bytes per k_sim_slots launch, source) from the small JSON that sits beside the committed
-    `ncu --set full` summary and names the table it was taken from, or (None, why)."""
+    `ncu --set full` summary and names its table, or (None, why) -- also when the simulator sources are
+    no longer the ones that were profiled (their SHA-256 is stamped in the file)."""
     path = os.path.join(ROOT, SIM_PROFILE)
     try:
         rec = json.load(open(path))
         total = float(rec["dram__bytes_read.sum"]) + float(rec["dram__bytes_write.sum"])
-        return total, f"{SIM_PROFILE}: {rec.get('table', '?')} (kernel source as of commit {rec.get('commit', '?')})"
+        if _sources_sha256(rec["source_files"]) != rec["source_sha256"]:
+            return None, f"{SIM_PROFILE} was captured from other simulator sources (commit {rec.get('commit', '?')}): capture again"
+        return total, f"{SIM_PROFILE}: {rec.get('table', '?')} (sources as of commit {rec.get('commit', '?')})"
     except (OSError, KeyError, ValueError):
         return None, f"{SIM_PROFILE} missing or unreadable"
 

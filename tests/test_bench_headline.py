@@ -80,5 +80,10 @@ def test_headline_refuses_a_missing_key_and_an_oversized_line():
 
 
 def test_committed_traffic_file_is_read():
+    """... and only while the simulator sources are the ones that were profiled (SHA-256 stamped in the file)."""
     total, src = bench.profiled_dram_traffic()
-    assert total == 237644544 + 152947712 and "r02_kslots_traffic.json" in src
+    rec = json.load(open(bench.os.path.join(bench.ROOT, bench.SIM_PROFILE)))
+    if bench._sources_sha256(rec["source_files"]) == rec["source_sha256"]:
+        assert total == rec["dram__bytes_read.sum"] + rec["dram__bytes_write.sum"] and bench.SIM_PROFILE in src
+    else:
+        assert total is None and "capture again" in src
