@@ -174,22 +174,22 @@ def trace_fingerprint(tr: "Trace") -> str:
 def admit_state(seed: int, n_wait: int, n_run: int, M: int, fill: float = 0.8):
     """Inputs of one stateless admission decision (bench.py's svf_admit sweep; BASELINE.json configs[3]
     laws for the waiting queue): waiting (s, o, a, bit) in arrival order and a running set (kv, rem)
-    whose remaining steps are uniform and whose held tokens are scaled so that the set alone peaks
-    at ``fill * M`` -- a loaded engine with room for a few more.  Input shaping only: sorting and
-    running sums of the generator's own draws, none of the method's decisions."""
+    with uniform remaining steps and lognormal held tokens, the tokens scaled down so that the final
+    footprints sum to at most ``fill * M``:  sum_j (kv_j + rem_j) <= fill * M.  A request never holds
+    more than kv + rem, so the set is feasible on its own whatever the order of completions -- a loaded
+    engine with room for a few more.  Input shaping only (two sums of the generator's own draws):
+    no key, no ordering by completion time, no feasibility check."""
     sd = instance_seed(88, seed)
     w_s = lognormal_int(sd, 2, 3, n_wait, 1000.0, 0.8, 16, 8192)
     w_o = lognormal_int(sd, 4, 5, n_wait, 400.0, 1.0, 1, 4096)
     w_a = np.sort(uniform_int(sd, 1, n_wait, 0, 5000))
     w_bit = (w_o > 400).astype(np.uint8)
-    rem_hi = int(max(8, min(3000, 1.6 * M / max(n_run, 1))))
+    rem_hi = int(max(8, min(3000, fill * M / max(n_run, 1))))      # mean rem = half of an equal share of fill * M
     r_rem = uniform_int(sd, 6, n_run, 1, rem_hi)
     r_kv = lognormal_int(sd, 7, 8, n_run, 1200.0, 0.8, 16, 12000)
     if n_run:
-        order = np.argsort(-r_rem, kind="stable")
-        cum = np.cumsum(r_kv[order].astype(np.int64)).astype(np.float64)
-        growth = (r_rem[order].astype(np.int64) * np.arange(1, n_run + 1)).astype(np.float64)
-        scale = float(np.clip(((fill * M - growth) / cum).min(), 0.0, 1.0))
+        room = fill * M - float(r_rem.astype(np.int64).sum())
+        scale = float(np.clip(room / float(r_kv.astype(np.int64).sum()), 0.0, 1.0))
         r_kv = np.maximum((r_kv * scale).astype(np.int32), 0)
     return w_s, w_o, w_a, w_bit, r_kv, r_rem
 

@@ -81,3 +81,5 @@ def test_admit_state_is_a_loaded_but_feasible_engine():
             order = np.argsort(-r_rem, kind="stable")
             peak = (np.cumsum(r_kv[order].astype(np.int64)) + r_rem[order].astype(np.int64) * np.arange(1, R + 1)).max()
             assert peak <= 0.8 * M + R
+            # ... which the generator guarantees through the final footprints alone (no completion-time formula in it)
+            assert int((r_kv.astype(np.int64) + r_rem).sum()) <= 0.8 * M or not r_kv.any()
