@@ -192,7 +192,8 @@ int svf_simulate_policies(const svf_trace_t* trace, int n_policies, const int* p
  * lb_out[j]; TEL(policy) * M / lb_out[j] upper-bounds the policy's approximation ratio where the
  * optimum cannot be computed.  Arrivals, `bit` and `output_key` are not read.  lb_out: [dev] [I]
  * int64; status_out: [dev] [I] int32 or NULL: SVF_OK, SVF_ERANGE (o_i < 1 or s_i < 0),
- * SVF_EOVERFLOW (some volume >= 2^32 -- the width rule of every key, R11 -- or bound >= 2^63),
+ * SVF_EOVERFLOW (bound >= 2^63; ALSO any volume >= 2^32: a limit of this library, whose presort
+ * orders 32-bit keys -- Eq. 5 itself sets no width and the CPU oracle returns the exact bound there, R19),
  * SVF_EINVAL (bad offsets); lb_out[j] = 0 unless SVF_OK.
  * Keys + the same presort as svf_simulate + one reduction kernel. */
 size_t svf_volume_lower_bound_workspace_bytes(const svf_trace_t* trace);
@@ -206,6 +207,12 @@ int svf_volume_lower_bound(const svf_trace_t* trace, int64_t* lb_out, int32_t* s
 size_t svf_sort_workspace_bytes(int64_t n, int bit_lo, int bit_hi);
 int svf_sort_words(int64_t n, const uint64_t* words_in, uint64_t* words_out, int bit_lo,
                    int bit_hi, void* ws, size_t ws_bytes, void* stream);
+
+/* For tests of the sizing rule (host only, no device needed): the bytes a call of
+ * svf_simulate_policies with THIS budget M carves from `ws` (M picks the kernel form, and the forms
+ * differ in scratch).  Always <= svf_simulate_policies_workspace_bytes(trace, n_policies), which is
+ * the maximum over every M and stays the size a caller must provide.  0 on bad arguments. */
+size_t svf_simulate_layout_bytes(const svf_trace_t* trace, int n_policies, int64_t M);
 
 /* Number of kernels the last call of each kind enqueued on this host thread (for the
  * "gpu_launches" count of bench.py); which: 0 = svf_keys, 1 = svf_admit, 2 = svf_simulate,

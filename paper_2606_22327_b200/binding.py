@@ -22,7 +22,7 @@ OK, EINVAL, EWORKSPACE, ECUDA = 0, 1, 2, 3
 ERANGE, EUNSORTED, EINFEASIBLE, EOVERFLOW = 16, 17, 18, 19
 
 EXPORTS = ("svf_keys", "svf_admit_workspace_bytes", "svf_admit", "svf_admit_static", "svf_simulate_workspace_bytes",
-           "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies",
+           "svf_simulate", "svf_simulate_policies_workspace_bytes", "svf_simulate_policies", "svf_simulate_layout_bytes",
            "svf_volume_lower_bound_workspace_bytes", "svf_volume_lower_bound", "svf_sort_workspace_bytes", "svf_sort_words", "svf_last_launch_count",
            "svf_status_string", "svf_version", "svf_set_profiling", "svf_simulate_phase_ms",
            "svf_simulate_work_counts", "svf_admit_phase_ms")
@@ -83,6 +83,8 @@ def lib():
         L.svf_simulate_policies.restype = C.c_int
         L.svf_simulate_policies.argtypes = [C.POINTER(_Trace), C.c_int, C.POINTER(C.c_int), C.c_int64,
                                             C.POINTER(_Result), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.svf_simulate_layout_bytes.restype = C.c_size_t
+        L.svf_simulate_layout_bytes.argtypes = [C.POINTER(_Trace), C.c_int, C.c_int64]
         L.svf_volume_lower_bound_workspace_bytes.restype = C.c_size_t
         L.svf_volume_lower_bound_workspace_bytes.argtypes = [C.POINTER(_Trace)]
         L.svf_volume_lower_bound.restype = C.c_int

@@ -385,6 +385,14 @@ struct SimConfig {
 constexpr size_t SMEM_STATE_LIMIT = 200 * 1024;
 constexpr size_t SMEM_WARP_STATE_LIMIT = 12 * 1024;   // one-warp groups: keep >= 16 CTAs per SM
 constexpr int SLOT_K = 16;                            // register slots per thread
+// The budget M reaches sim_config through ONE estimate, r_est = min(max_instance, M / 512) running
+// requests, and through M >= 2^30 (the wide kernel).  r_est is only ever compared with these four
+// breakpoints, so one probe per class of r_est (at most a break, just above each) plus one wide M
+// visits every kernel form a trace can get: sim_workspace_bytes sizes for the largest of them.
+constexpr int64_t R_EST_TOKENS = 512;
+constexpr int64_t R_EST_WARP = 32 * SLOT_K, R_EST_WARP_SPARE = 48 * SLOT_K, R_EST_WARP32 = 100 * SLOT_K,
+                  R_EST_CTA256 = 128 * SLOT_K;
+constexpr int64_t R_EST_BREAKS[4] = {R_EST_WARP, R_EST_WARP_SPARE, R_EST_WARP32, R_EST_CTA256};
 
 SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
 {
@@ -407,17 +415,17 @@ SimConfig sim_config(const svf_trace_t* tr, int64_t M, int P = 1)
     int64_t w = I > 0 ? target_warps / (I * (P > 0 ? P : 1)) : 1;   // P policies share one launch
     int threads = 32;
     if (c.slots) {
-        const int64_t r_est = mx < M / 512 ? mx : M / 512;
+        const int64_t r_est = mx < M / R_EST_TOKENS ? mx : M / R_EST_TOKENS;
         // (an estimate just above the warp's 512 slots -- configs[2]: 585, peaks of 530 -- is served better by
         // the warp and a few ext slots unless warps are plentiful; far above it the CTA wins even at w = 2)
         // and the register-queue warp kernel (instances up to 2,048 requests) beats the CTA at any w
         const bool regq = mx <= QREG_RANKS * QREG_MAX_WORDS;
-        if ((r_est > 32 * SLOT_K && w >= 4 && !regq) || (r_est > 48 * SLOT_K && w >= 2)) threads = 128;
-        if (r_est > 128 * SLOT_K && w >= 8) threads = 256;
+        if ((r_est > R_EST_WARP && w >= 4 && !regq) || (r_est > R_EST_WARP_SPARE && w >= 2)) threads = 128;
+        if (r_est > R_EST_CTA256 && w >= 8) threads = 256;
         // ... unless ONE warp with 32 slots per thread holds the set (estimates up to 1,600: the estimate
         // counts 512 tokens per running request, real sets are smaller): no barrier, no scalar part
         // replicated in four warps (configs[4] at M = 800k: 10.4 ms with CTAs)
-        if (threads == 128 && r_est <= 100 * SLOT_K) { threads = 32; c.k = 32; }
+        if (threads == 128 && r_est <= R_EST_WARP32) { threads = 32; c.k = 32; }
     } else {
         while (threads < 1024 && (threads * 2) / 32 <= w && threads * 4 <= mx) threads *= 2;
         if (threads == 64) threads = 128;
@@ -596,20 +604,34 @@ using namespace svf;
 namespace svf {
 namespace {
 
+// bytes a call with budget M lays out, with as many global slots as the launch can have CTAs
+size_t sim_layout_bytes_at(const svf_trace_t* tr, int P, int64_t M)
+{
+    SimConfig c = sim_config(tr, M, P);
+    SimWs w;
+    int64_t slots = c.gslot_bytes ? (int64_t)c.max_cta_per_sm * sm_count() : 0;
+    if (slots > tr->n_instances * P) slots = tr->n_instances * P;
+    sim_ws_layout(&w, nullptr, tr, c, (int)slots, P);
+    return w.total;
+}
+
+bool sim_ws_args_ok(const svf_trace_t* tr, int P)
+{
+    return tr && tr->n_instances >= 0 && tr->n_requests >= 0 && tr->max_instance >= 0 && P >= 1 && P <= MAX_POLICIES;
+}
+
 size_t sim_workspace_bytes(const svf_trace_t* tr, int P)
 {
-    if (!tr || tr->n_instances < 0 || tr->n_requests < 0 || tr->max_instance < 0 || P < 1 || P > MAX_POLICIES) return 0;
-    // M is not known here and picks the kernel family (through min(max_instance, M / 512) against the
-    // register-slot capacities 512 and 2048, and through M >= 2^30): size for the largest layout
-    size_t need = 0;
-    for (int64_t M : {(int64_t)0, (int64_t)512 * 600, (int64_t)512 * 3000, (int64_t)1 << 30}) {
-        SimConfig c = sim_config(tr, M, P);
-        SimWs w;
-        int64_t slots = c.gslot_bytes ? (int64_t)c.max_cta_per_sm * sm_count() : 0;
-        if (slots > tr->n_instances * P) slots = tr->n_instances * P;
-        sim_ws_layout(&w, nullptr, tr, c, (int)slots, P);
-        need = w.total > need ? w.total : need;
+    if (!sim_ws_args_ok(tr, P)) return 0;
+    // M is not known here and picks the kernel family: size for the largest layout over one probe per
+    // class of r_est (see R_EST_BREAKS) and one wide budget
+    size_t need = sim_layout_bytes_at(tr, P, 0);
+    for (int64_t brk : R_EST_BREAKS) {
+        const size_t b = sim_layout_bytes_at(tr, P, R_EST_TOKENS * (brk + 1));
+        need = b > need ? b : need;
     }
+    const size_t wide = sim_layout_bytes_at(tr, P, (int64_t)1 << 30);
+    need = wide > need ? wide : need;
     return need + 256;
 }
 
@@ -815,6 +837,12 @@ extern "C" size_t svf_simulate_workspace_bytes(const svf_trace_t* tr) { return s
 extern "C" size_t svf_simulate_policies_workspace_bytes(const svf_trace_t* tr, int n_policies)
 {
     return sim_workspace_bytes(tr, n_policies);
+}
+
+extern "C" size_t svf_simulate_layout_bytes(const svf_trace_t* tr, int n_policies, int64_t M)
+{
+    if (!sim_ws_args_ok(tr, n_policies) || M < 0) return 0;
+    return sim_layout_bytes_at(tr, n_policies, M) + 256;
 }
 
 extern "C" int svf_simulate(const svf_trace_t* tr, int policy, int64_t M, const svf_result_t* out,

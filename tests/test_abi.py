@@ -250,3 +250,35 @@ def test_static_admit_checks_arguments_and_its_size_limit_on_the_host(svf_lib):
     L.svf_admit_workspace_bytes.argtypes = [C.c_int64, C.c_int64]
     assert (mw, mr) == (65536, 8192)
     assert L.svf_admit_workspace_bytes(mw, mr) <= sh << 20
+
+
+def test_simulate_workspace_covers_the_layout_of_every_budget(svf_lib):
+    """svf_simulate*_workspace_bytes is taken without knowing M, yet M picks the kernel form and the forms
+    carve different scratch.  Sweep M (around every breakpoint of the group-width rule, 512 tokens per
+    estimated running request, and across 2^30), instance sizes around every state-placement limit,
+    instance counts from one to many waves and 1 / 4 / 8 policies: no budget may need more than the
+    size the caller was told to provide."""
+    from paper_2606_22327_b200 import binding
+    L = svf_lib
+    L.svf_simulate_policies_workspace_bytes.restype = C.c_size_t
+    L.svf_simulate_policies_workspace_bytes.argtypes = [C.POINTER(binding._Trace), C.c_int]
+    L.svf_simulate_layout_bytes.restype = C.c_size_t
+    L.svf_simulate_layout_bytes.argtypes = [C.POINTER(binding._Trace), C.c_int, C.c_int64]
+    budgets = [0, 1, 511, 512, 2 ** 30 - 1, 2 ** 30, 2 ** 30 + 1, 2 ** 40]
+    for r in (511, 512, 513, 767, 768, 769, 1023, 1024, 1025, 1599, 1600, 1601, 2047, 2048, 2049, 4096, 8192, 8193, 100_000):
+        budgets += [512 * r - 1, 512 * r, 512 * r + 511, 512 * (r + 1)]
+    checked = 0
+    for mx in (1, 31, 33, 500, 1000, 1024, 1025, 2048, 2049, 4096, 4097, 8192, 8193, 20_000, 200_000):
+        for I in (1, 2, 7, 148, 1000, 4096, 100_000):
+            N = min(I * mx, 2 ** 29)
+            for P in (1, 4, 8):
+                tr = binding._Trace()
+                tr.n_instances, tr.n_requests, tr.max_instance = I, N, min(mx, N)
+                cap = L.svf_simulate_policies_workspace_bytes(C.byref(tr), P)
+                assert cap > 0
+                for M in budgets:
+                    need = L.svf_simulate_layout_bytes(C.byref(tr), P, M)
+                    assert 0 < need <= cap, f"max_instance {mx}, I {I}, P {P}, M {M}: layout {need} > workspace {cap}"
+                    checked += 1
+    assert checked > 20_000
+    assert L.svf_simulate_layout_bytes(None, 1, 0) == 0 and L.svf_simulate_layout_bytes(C.byref(tr), 9, 0) == 0
