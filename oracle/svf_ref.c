@@ -411,9 +411,12 @@ int svf_ref_simulate(int64_t n_instances, const int64_t *offsets, const int32_t 
  * NEXT-2: the volume lower bound of Proposition 3.1 (Eq. 5) for burst input,
  *     M * TEL(OPT) >= LB = sum_{j=1..N} sum_{i=1..j} vol_(i),   vol_(1) <= ... <= vol_(N),
  * written as printed: sort the volumes (Eq. 1), then for every j add the sum of the first j.
- * lb_out[j] = LB of instance j (int64); status_out[j] = ST_EOVERFLOW if LB >= 2^63 or some volume
- * >= 2^32 (lb 0; R11: the width rule of every key), ST_ERANGE if some o < 1 or s < 0 (wins).  Arrivals are not looked at: the bound is about the burst
- * version of the instance.
+ * lb_out[j] = LB of instance j (int64); status_out[j] = ST_EOVERFLOW only if LB itself does not fit
+ * (LB >= 2^63; lb 0), ST_ERANGE if some o < 1 or s < 0 (wins).  Eq. 5 is a statement about integers
+ * and sets no width: a single volume may be anything an int64 holds (s, o < 2^31 gives < 2^62.6);
+ * the sums are carried in 128 bits.  (The CUDA library refuses instances that hold a volume >= 2^32
+ * -- its presort orders 32-bit keys, R19 -- that is ITS limit, not the bound's.)
+ * Arrivals are not looked at: the bound is about the burst version of the instance.
  * ---------------------------------------------------------------------------------------- */
 int svf_ref_volume_lower_bound(int64_t n_instances, const int64_t *offsets, const int32_t *prompt,
                                const int32_t *output, int64_t *lb_out, int32_t *status_out)
@@ -425,9 +428,7 @@ int svf_ref_volume_lower_bound(int64_t n_instances, const int64_t *offsets, cons
         int64_t *vol = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
         for (int64_t i = 0; i < n; ++i) {
             if (output[lo + i] < 1 || prompt[lo + i] < 0) st = ST_ERANGE;
-            vol[i] = ref_key(POL_SVF, prompt[lo + i], output[lo + i], 0, 0, 0, 0);
-            /* a volume is an SVF key: keys >= 2^32 are ST_EOVERFLOW at every entry point (reading R11) */
-            if (st == ST_OK && vol[i] >= ((int64_t)1 << 32)) st = ST_EOVERFLOW;
+            vol[i] = ref_key(POL_SVF, prompt[lo + i], output[lo + i], 0, 0, 0, 0);   /* Eq. 1, exact in int64 */
         }
         unsigned __int128 lb = 0, prefix = 0;
         if (st == ST_OK) {

@@ -159,16 +159,24 @@ def test_volume_lower_bound_closed_forms(oracle):
     bad = T.random_small(3, 5, 9, 9, 50)
     bad.output[2] = 0
     assert int(oracle.volume_lower_bound(bad)[1][0]) == oracle.ERANGE
-    # a volume is an SVF key: >= 2^32 is EOVERFLOW at every entry point (reading R11), the same rule as
-    # in keys / simulate.  s = o = 60,000: 60000^2 + 60000*60001/2 = 5,400,030,000 >= 2^32 = 4,294,967,296;
-    # s = 30,000, o = 60,000: 3,600,030,000 < 2^32
+    # Eq. 5 sets no width on a volume: the bound is exact also where a volume passes 2^32 (a width the
+    # CUDA library's 32-bit presort keys refuse, R19 -- its limit, tested on the GPU side).  By hand:
+    # s = o = 60,000: 60000^2 + 60000*60001/2 = 5,400,030,000 >= 2^32 = 4,294,967,296;
+    # s = 30,000, o = 60,000: 3,600,030,000;  LB = 2 * 3,600,030,000 + 5,400,030,000 = 12,600,090,000
     below = T._one("below", np.zeros(2, np.int32), np.array([30_000, 30_000]), np.array([60_000, 60_000]), np.zeros(2, np.uint8), 10 ** 9, 1, 1)
     lb, st = oracle.volume_lower_bound(below)
     assert int(st[0]) == 0 and int(lb[0]) == 3 * 3_600_030_000
     mixed = T._one("mixed", np.zeros(2, np.int32), np.array([60_000, 30_000]), np.array([60_000, 60_000]), np.zeros(2, np.uint8), 10 ** 9, 1, 1)
     lb, st = oracle.volume_lower_bound(mixed)
-    assert int(st[0]) == oracle.EOVERFLOW and int(lb[0]) == 0
-    assert oracle.keys(oracle.SVF, mixed.prompt, mixed.output)[0] == oracle.EOVERFLOW       # the same rule
+    assert int(st[0]) == 0 and int(lb[0]) == 12_600_090_000
+    assert oracle.keys(oracle.SVF, mixed.prompt, mixed.output)[0] == oracle.EOVERFLOW       # as a KEY it is still refused (R11)
+    # the largest requests the arrays can hold: volumes near 2^62.6, two of them still fit, five do not
+    big = lambda n: T._one("big", np.zeros(n, np.int32), np.full(n, 2 ** 31 - 1), np.full(n, 2 ** 31 - 1), np.zeros(n, np.uint8), 10 ** 9, 1, 1)
+    v = (2 ** 31 - 1) ** 2 + ((2 ** 31 - 1) ** 2 + (2 ** 31 - 1)) // 2
+    lb, st = oracle.volume_lower_bound(big(1))
+    assert int(st[0]) == 0 and int(lb[0]) == v
+    lb, st = oracle.volume_lower_bound(big(5))                                          # 15 v >= 2^63
+    assert 15 * v >= 2 ** 63 and int(st[0]) == oracle.EOVERFLOW and int(lb[0]) == 0
 
 
 def test_volume_lower_bound_bounds_every_schedule_and_the_optimum(oracle):
