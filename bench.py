@@ -581,8 +581,9 @@ def admit_sweep(B, torch, dev, peak):
     M = 1e6, policy SVF; the phase split comes from CUDA events the library records on the stream."""
     res = []
     M = 1_000_000
-    for W in (1 << 10, 1 << 14, 1 << 18):
-        for R in (256, 1024, 4096):
+    for W, runs in ((1 << 10, (256, 1024, 4096)), (1 << 14, (256, 1024, 4096)), (1 << 18, (256, 1024, 4096)),
+                    (1 << 20, (1024,)), (1 << 22, (1024,))):         # the last two: queues beyond L2, where bandwidth starts to count
+        for R in runs:
             w_s, w_o, w_a, w_bit, r_kv, r_rem = T.admit_state(W + R, W, R, M)
             d = [torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in (w_s, w_o, w_a, w_bit, r_kv, r_rem)]
             ws = torch.empty(B.svf_admit_workspace_bytes(W, R), dtype=torch.uint8, device=dev)
@@ -609,7 +610,10 @@ def admit_sweep(B, torch, dev, peak):
                                      "whole_call_under_events": float(ph[3])},
                         # at these sizes the call is a short chain of small launches (or one CTA): latency, not
                         # bandwidth, sets the time; the bytes are reported as a rate, without an HBM fraction
-                        "roofline": {"bound": "latency", "achieved": algo / ms / 1e6, "unit": "GB/s", "algorithmic_bytes": algo,
+                        "roofline": {"bound": "hbm", "achieved": algo / ms / 1e6, "peak": peak, "unit": "GB/s", "frac": algo / ms / 1e6 / peak,
+                                     "algorithmic_bytes": algo, "note": "queue beyond L2: keys + four onesweep passes over the whole queue set the time"}
+                                    if W >= 1 << 20 else
+                                    {"bound": "latency", "achieved": algo / ms / 1e6, "unit": "GB/s", "algorithmic_bytes": algo,
                                      "note": ("one launch, one CTA: validation, keys, both sorts and the bisection in shared memory (the phase "
                                               "split does not apply: all under 'admission'); bound by one SM's issue rate and barriers") if fused else
                                              "a chain of 13 small launches: launch latency, not bandwidth, sets the time at these sizes"}})
