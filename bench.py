@@ -598,13 +598,32 @@ def admit_sweep(B, torch, dev, peak):
             B.set_profiling(False)
             ph = np.array(ph).mean(axis=0)
             k = int(out.n_admitted.item())
+            # a deep call is a chain of 13 small launches: the same call captured once in a CUDA graph and
+            # replayed (what a caller that decides every engine step would do); same buffers, same answer
+            graph_ms = None
+            if W + R > 8192:
+                try:
+                    side = torch.cuda.Stream(device=dev)
+                    with torch.cuda.stream(side):
+                        call()
+                    torch.cuda.synchronize()
+                    graph = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(graph, stream=side):
+                        call()
+                    out.n_admitted.fill_(-1)
+                    graph_ms = _time_cuda(torch, graph.replay, reps=10)
+                    if int(out.n_admitted.item()) != k:
+                        graph_ms = f"replay gave {int(out.n_admitted.item())} admitted, the direct call {k}"
+                    del graph
+                except Exception as e:      # an extra: recorded, never fatal
+                    graph_ms = f"{type(e).__name__}: {e}"
             # what the call must move: validation + keys read s, o, a (12 B) and write the packed word
             # (8 B); the sort reads the words once for its histograms and reads + writes them once per
             # executed pass (26-bit keys: four 8-bit passes over [32, 64)); the sorted words are copied
             # out (16 B); the admission reads the running set and the first candidates (12 B each)
             fused = W + R <= 8192          # the library then takes the whole decision in ONE launch on one CTA
             algo = (W * (12 + 8 + 4) + R * 8) if fused else W * (12 + 8 + 8 + 16 * 4 + 16) + (R + min(W, 8192 - R)) * 12
-            res.append({"W": W, "R": R, "ms": ms, "admitted": k, "launches": B.last_launch_count(1),
+            res.append({"W": W, "R": R, "ms": ms, "ms_replayed_from_a_cuda_graph": graph_ms, "admitted": k, "launches": B.last_launch_count(1),
                         "decisions_per_sec": (k + 1) / ms * 1e3, "queue_entries_per_sec": W / ms * 1e3,
                         "phase_ms": {"keys_and_validation": float(ph[0]), "sorts": float(ph[1]), "admission": float(ph[2]),
                                      "whole_call_under_events": float(ph[3])},
