@@ -87,3 +87,29 @@ def test_committed_traffic_file_is_read():
         assert total == rec["dram__bytes_read.sum"] + rec["dram__bytes_write.sum"] and bench.SIM_PROFILE in src
     else:
         assert total is None and "capture again" in src
+
+
+def test_reference_arm_prints_one_short_strict_json_line_on_a_cpu_box():
+    """`bench.py --impl reference` is the driver's other arm: the oracle on the host cores, no GPU.  Run it
+    on a small batch as the driver would (a subprocess), and read its last stdout line the same way."""
+    import os
+    import subprocess
+    import sys
+    r = subprocess.run([sys.executable, os.path.join(bench.ROOT, "bench.py"), "--impl", "reference", "--instances", "8",
+                        "--requests", "60", "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    last = r.stdout.strip().splitlines()[-1]
+    assert len(last.encode()) <= 4096
+
+    def no_constants(name):
+        raise AssertionError(f"non-strict JSON constant {name}")
+    line = json.loads(last, parse_constant=no_constants)
+    assert line["impl"] == "reference" and line["metric"] == bench.METRIC and line["unit"] == bench.UNIT
+    assert line["value"] > 0 and line["steps"] == 2 and line["gpu_launches"] == 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"]
+    assert line["e2e"] == {"value": line["value"], "unit": bench.UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    # under torchrun every rank but 0 exits 0 without work and without output
+    r1 = subprocess.run([sys.executable, os.path.join(bench.ROOT, "bench.py"), "--impl", "reference", "--instances", "8",
+                         "--requests", "60", "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=300,
+                        env=dict(os.environ, RANK="1", WORLD_SIZE="2"))
+    assert r1.returncode == 0 and r1.stdout.strip() == ""
